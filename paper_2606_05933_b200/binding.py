@@ -1,0 +1,187 @@
+"""ctypes binding of libslidingattn.so (include/slidingattn.h).  Argument marshalling only: every step of
+the path runs in the CUDA kernels.  There is no CPU fallback — if the compiled library is missing or no
+sm_100 device is present the calls raise."""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+from typing import Optional
+
+import numpy as np
+import torch
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libslidingattn.so"
+_lib = None
+
+SS_OK = 0
+EXPORTS = ["ss_version", "ss_status_string", "ss_last_error_string", "ss_create", "ss_destroy",
+           "ss_workspace_bytes", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
+           "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path"]
+
+
+class ss_config(ctypes.Structure):
+    _fields_ = [("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32),
+                ("head_dim", ctypes.c_int32), ("page_size", ctypes.c_int32),
+                ("num_pages", ctypes.c_int64), ("max_requests", ctypes.c_int32),
+                ("max_tokens", ctypes.c_int32), ("max_pages_per_req", ctypes.c_int32)]
+
+
+class ss_work_item(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in
+                ("kind", "req", "head", "row0", "nrows", "kv_begin", "kv_end", "split", "nsplit",
+                 "partial", "q_pos0", "reserved")]
+
+
+WORK_ITEM_DTYPE = np.dtype([(n, np.int32) for n, _ in ss_work_item._fields_])
+
+
+class SlidingAttnError(RuntimeError):
+    pass
+
+
+def load():
+    """dlopen the in-tree library; raises (never falls back) if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise SlidingAttnError(f"{LIB_PATH} not built: run `python -m paper_2606_05933_b200.build` "
+                               "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = ctypes.CDLL(str(LIB_PATH))
+    vp, i32, f32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_float
+    lib.ss_version.restype = ctypes.c_int
+    lib.ss_status_string.restype = ctypes.c_char_p
+    lib.ss_status_string.argtypes = [ctypes.c_int]
+    lib.ss_last_error_string.restype = ctypes.c_char_p
+    lib.ss_last_error_string.argtypes = [vp]
+    lib.ss_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(ss_config), vp, vp]
+    lib.ss_destroy.argtypes = [vp]
+    lib.ss_workspace_bytes.argtypes = [vp]
+    lib.ss_workspace_bytes.restype = ctypes.c_size_t
+    lib.ss_kv_append.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, vp]
+    lib.ss_mixed_attention.argtypes = [vp, vp, vp, vp, vp, i32, i32, f32, vp, vp, vp, ctypes.c_size_t, vp]
+    lib.ss_build_worklist.argtypes = [vp, vp, vp, i32, i32, vp, ctypes.c_size_t, vp, i32,
+                                      ctypes.POINTER(i32 * 3), vp]
+    lib.ss_iteration_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
+    lib.ss_last_launch_count.argtypes = [vp]
+    lib.ss_debug_force_simple_path.argtypes = [vp, ctypes.c_int]
+    for name in ("ss_create", "ss_destroy", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
+                 "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path"):
+        getattr(lib, name).restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream or None
+
+
+class SlidingAttn:
+    """Handle bound to one pair of paged caches [num_pages, Hkv, 16, D] bf16 on the current device."""
+
+    def __init__(self, num_q_heads: int, num_kv_heads: int, head_dim: int, k_cache: torch.Tensor,
+                 v_cache: torch.Tensor, max_requests: int, max_tokens: int, max_pages_per_req: int):
+        self.lib = load()
+        if not (k_cache.is_cuda and v_cache.is_cuda):
+            raise SlidingAttnError("caches must be CUDA tensors (no CPU path exists)")
+        assert k_cache.dtype == torch.bfloat16 and k_cache.is_contiguous() and k_cache.shape == v_cache.shape
+        P, Hkv, page, D = k_cache.shape
+        assert Hkv == num_kv_heads and D == head_dim
+        self.cfg = ss_config(num_q_heads, num_kv_heads, head_dim, page, P, max_requests, max_tokens,
+                             max_pages_per_req)
+        self.k_cache, self.v_cache = k_cache, v_cache
+        self._h = ctypes.c_void_p()
+        self._check(self.lib.ss_create(ctypes.byref(self._h), ctypes.byref(self.cfg), k_cache.data_ptr(),
+                                       v_cache.data_ptr()), create=True)
+        self.workspace_bytes = int(self.lib.ss_workspace_bytes(self._h))
+        self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=k_cache.device)
+
+    def _check(self, rc: int, create: bool = False):
+        if rc != SS_OK:
+            detail = b"" if create or not self._h else self.lib.ss_last_error_string(self._h)
+            raise SlidingAttnError(f"{self.lib.ss_status_string(rc).decode()} ({rc}) {detail.decode()}")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.ss_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- the two calls of the path -------------------------------------------------------------
+    def kv_append(self, k_new, v_new, block_table, query_start_loc, ctx_lens, stream=None):
+        R, T = ctx_lens.shape[0], k_new.shape[0]
+        self._check(self.lib.ss_kv_append(self._h, _ptr(k_new), _ptr(v_new), _ptr(block_table),
+                                          _ptr(query_start_loc), _ptr(ctx_lens), R, T, _stream_ptr(stream)))
+
+    def mixed_attention(self, q, block_table, query_start_loc, ctx_lens, scale, out=None, lse=None,
+                        stream=None):
+        R, T = ctx_lens.shape[0], q.shape[0]
+        if out is None:
+            out = torch.empty_like(q)
+        self._check(self.lib.ss_mixed_attention(self._h, _ptr(q), _ptr(block_table), _ptr(query_start_loc),
+                                                _ptr(ctx_lens), R, T, float(scale), _ptr(out), _ptr(lse),
+                                                self.workspace.data_ptr(), self.workspace_bytes,
+                                                _stream_ptr(stream)))
+        return out
+
+    # ---- aids ----------------------------------------------------------------------------------
+    def build_worklist(self, query_start_loc, ctx_lens, stream=None):
+        R = ctx_lens.shape[0]
+        T = int(self.cfg.max_tokens)
+        counts = (ctypes.c_int32 * 3)()
+        self._check(self.lib.ss_build_worklist(self._h, _ptr(query_start_loc), _ptr(ctx_lens), R, T,
+                                               self.workspace.data_ptr(), self.workspace_bytes, None, 0,
+                                               ctypes.byref(counts), _stream_ptr(stream)))
+        n = counts[0] + counts[1]
+        items = np.zeros(n, dtype=WORK_ITEM_DTYPE)
+        if n:
+            self._check(self.lib.ss_build_worklist(self._h, _ptr(query_start_loc), _ptr(ctx_lens), R, T,
+                                                   self.workspace.data_ptr(), self.workspace_bytes,
+                                                   items.ctypes.data, n, ctypes.byref(counts),
+                                                   _stream_ptr(stream)))
+        return items, tuple(counts)
+
+    def iteration_host(self, q, k_new, v_new, block_table, query_start_loc, ctx_lens, scale, out, stream=None):
+        """Host (pinned) tensors in, host tensor out; H2D + append + attention + D2H + sync inside."""
+        R, T = ctx_lens.shape[0], q.shape[0]
+        self._check(self.lib.ss_iteration_host(self._h, _ptr(q), _ptr(k_new), _ptr(v_new), _ptr(block_table),
+                                               _ptr(query_start_loc), _ptr(ctx_lens), R, T, float(scale),
+                                               _ptr(out), _stream_ptr(stream)))
+        return out
+
+    def last_launch_count(self) -> int:
+        return int(self.lib.ss_last_launch_count(self._h))
+
+    def force_simple_path(self, on: bool):
+        self._check(self.lib.ss_debug_force_simple_path(self._h, int(on)))
+
+
+def kv_append(handle: SlidingAttn, k_new, v_new, block_table, query_start_loc, ctx_lens, stream=None):
+    """north_star kv_append(k_new, v_new, block_table, slot offsets): slot offsets = ctx_lens + query_start_loc."""
+    return handle.kv_append(k_new, v_new, block_table, query_start_loc, ctx_lens, stream)
+
+
+def mixed_attention(handle: SlidingAttn, q, block_table, query_start_loc, ctx_lens, scale, out=None,
+                    lse=None, stream=None):
+    """north_star mixed_attention(q, k_cache, v_cache, block_table, query_start_loc, ctx_lens, scale, out);
+    the caches are the ones the handle was created on."""
+    return handle.mixed_attention(q, block_table, query_start_loc, ctx_lens, scale, out, lse, stream)
+
+
+def handle_for(batch, tensors, extra_tokens: int = 0) -> SlidingAttn:
+    """Convenience: a handle sized for one workloads.Batch."""
+    return SlidingAttn(batch.num_q_heads, batch.num_kv_heads, batch.head_dim, tensors.k_cache, tensors.v_cache,
+                       max_requests=max(batch.R, 1), max_tokens=max(batch.T + extra_tokens, 1),
+                       max_pages_per_req=batch.max_pages_per_req)

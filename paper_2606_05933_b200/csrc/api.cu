@@ -1,0 +1,285 @@
+// C ABI of libslidingattn (include/slidingattn.h): argument checks, handle, launch sequencing.
+// No arithmetic of the method lives here; every step of the path runs in the kernels.
+#include <new>
+#include <string.h>
+
+#include "common.cuh"
+
+using namespace ss;
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    }
+    return fn;
+}
+
+bool aligned16(const void* p) { return (((uintptr_t)p) & 15u) == 0; }
+
+int fail_cuda(Handle* h, cudaError_t e, const char* where) {
+    if (h) snprintf(h->err, sizeof h->err, "%s: %s", where, cudaGetErrorString(e));
+    return SS_ERR_CUDA;
+}
+
+#define SS_CUDA(h, call, where)                                  \
+    do {                                                         \
+        cudaError_t e__ = (call);                                \
+        if (e__ != cudaSuccess) return fail_cuda(h, e__, where); \
+    } while (0)
+
+// KV cache viewed as a 2-D bf16 matrix [num_pages*Hkv*16 rows][D]; one TMA box = one page slab half:
+// 16 rows x 64 columns (128 bytes, SWIZZLE_128B), the canonical K-major UMMA / ldmatrix atom.
+int encode_cache_map(Handle* h, CUtensorMap* map, void* base) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) {
+        snprintf(h->err, sizeof h->err, "cuTensorMapEncodeTiled entry point not found");
+        return SS_ERR_CUDA;
+    }
+    const ss_config& c = h->cfg;
+    cuuint64_t gdim[2] = {(cuuint64_t)c.head_dim, (cuuint64_t)c.num_pages * c.num_kv_heads * kPage};
+    cuuint64_t gstride[1] = {(cuuint64_t)c.head_dim * 2};
+    cuuint32_t box[2] = {64u, (cuuint32_t)kPage};
+    cuuint32_t estr[2] = {1u, 1u};
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, gdim, gstride, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(h->err, sizeof h->err, "cuTensorMapEncodeTiled failed: %d", (int)r);
+        return SS_ERR_CUDA;
+    }
+    return SS_OK;
+}
+
+int check_batch_args(const Handle* h, const void* a, const void* b, const void* c, const void* d, int R, int T) {
+    if (!h) return SS_ERR_INVALID_ARG;
+    if (R < 0 || T < 0 || R > h->cfg.max_requests || T > h->cfg.max_tokens) return SS_ERR_INVALID_ARG;
+    if (R == 0 || T == 0) return SS_OK;
+    if (!a || !b || !c || !d) return SS_ERR_INVALID_ARG;
+    if (!aligned16(a) || !aligned16(b)) return SS_ERR_INVALID_ARG;
+    if ((((uintptr_t)c) & 3u) || (((uintptr_t)d) & 3u)) return SS_ERR_INVALID_ARG;
+    return SS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ss_version(void) { return SS_VERSION; }
+
+const char* ss_status_string(int s) {
+    switch (s) {
+        case SS_OK: return "SS_OK";
+        case SS_ERR_INVALID_ARG: return "SS_ERR_INVALID_ARG";
+        case SS_ERR_WORKSPACE_TOO_SMALL: return "SS_ERR_WORKSPACE_TOO_SMALL";
+        case SS_ERR_UNSUPPORTED_DEVICE: return "SS_ERR_UNSUPPORTED_DEVICE";
+        case SS_ERR_CUDA: return "SS_ERR_CUDA";
+        case SS_ERR_NOT_IMPLEMENTED: return "SS_ERR_NOT_IMPLEMENTED";
+        default: return "SS_ERR_UNKNOWN";
+    }
+}
+
+const char* ss_last_error_string(const ss_handle* hh) {
+    const Handle* h = (const Handle*)hh;
+    return h ? h->err : "null handle";
+}
+
+int ss_create(ss_handle** out_handle, const ss_config* cfg, void* k_cache, void* v_cache) {
+    if (!out_handle) return SS_ERR_INVALID_ARG;
+    *out_handle = nullptr;
+    if (!cfg || !k_cache || !v_cache || !aligned16(k_cache) || !aligned16(v_cache)) return SS_ERR_INVALID_ARG;
+    if (cfg->page_size != kPage) return SS_ERR_INVALID_ARG;
+    if (cfg->head_dim != 64 && cfg->head_dim != 128) return SS_ERR_INVALID_ARG;
+    if (cfg->num_q_heads <= 0 || cfg->num_kv_heads <= 0 || cfg->num_q_heads % cfg->num_kv_heads) return SS_ERR_INVALID_ARG;
+    if (cfg->num_q_heads / cfg->num_kv_heads > kMaxGroup) return SS_ERR_INVALID_ARG;
+    if (cfg->num_pages <= 0 || cfg->max_requests <= 0 || cfg->max_requests > 2048 || cfg->max_tokens <= 0 ||
+        cfg->max_pages_per_req <= 0)
+        return SS_ERR_INVALID_ARG;
+    if ((int64_t)cfg->max_pages_per_req * kPage > (int64_t)1 << 30) return SS_ERR_INVALID_ARG;
+
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return SS_ERR_CUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return SS_ERR_CUDA;
+    if (prop.major != 10) return SS_ERR_UNSUPPORTED_DEVICE;
+
+    Handle* h = new (std::nothrow) Handle();
+    if (!h) return SS_ERR_CUDA;
+    memset(h, 0, sizeof *h);
+    h->cfg = *cfg;
+    h->device = dev;
+    h->num_sms = prop.multiProcessorCount;
+    h->group = cfg->num_q_heads / cfg->num_kv_heads;
+    h->k_cache = k_cache;
+    h->v_cache = v_cache;
+    h->ws = workspace_layout(h->cfg, h->num_sms);
+    int rc = encode_cache_map(h, &h->tmap_k, k_cache);
+    if (rc == SS_OK) rc = encode_cache_map(h, &h->tmap_v, v_cache);
+    if (rc != SS_OK) {
+        delete h;
+        return rc;
+    }
+    h->have_tmaps = true;
+    *out_handle = (ss_handle*)h;
+    return SS_OK;
+}
+
+int ss_destroy(ss_handle* hh) {
+    Handle* h = (Handle*)hh;
+    if (!h) return SS_ERR_INVALID_ARG;
+    void* bufs[] = {h->st_q, h->st_knew, h->st_vnew, h->st_out, h->st_ws, h->st_bt, h->st_qsl, h->st_ctx};
+    for (void* b : bufs)
+        if (b) cudaFree(b);
+    delete h;
+    return SS_OK;
+}
+
+size_t ss_workspace_bytes(const ss_handle* hh) {
+    const Handle* h = (const Handle*)hh;
+    return h ? h->ws.total : 0;
+}
+
+int ss_last_launch_count(const ss_handle* hh) {
+    const Handle* h = (const Handle*)hh;
+    return h ? h->last_launches : 0;
+}
+
+int ss_debug_force_simple_path(ss_handle* hh, int on) {
+    Handle* h = (Handle*)hh;
+    if (!h) return SS_ERR_INVALID_ARG;
+    h->force_simple = on ? 1 : 0;
+    return SS_OK;
+}
+
+int ss_kv_append(ss_handle* hh, const void* k_new, const void* v_new, const int32_t* block_table,
+                 const int32_t* query_start_loc, const int32_t* ctx_lens, int32_t R, int32_t T, void* cuda_stream) {
+    Handle* h = (Handle*)hh;
+    int rc = check_batch_args(h, k_new, v_new, query_start_loc, ctx_lens, R, T);
+    if (rc != SS_OK) return rc;
+    h->last_launches = 0;
+    if (R == 0 || T == 0) return SS_OK;
+    if (!block_table || (((uintptr_t)block_table) & 3u)) return SS_ERR_INVALID_ARG;
+    SS_CUDA(h, launch_kv_append(h, k_new, v_new, block_table, query_start_loc, ctx_lens, R, T, (cudaStream_t)cuda_stream),
+            "kv_append launch");
+    h->last_launches = 1;
+    return SS_OK;
+}
+
+int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table, const int32_t* query_start_loc,
+                       const int32_t* ctx_lens, int32_t R, int32_t T, float scale, void* out, float* lse_or_null,
+                       void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    Handle* h = (Handle*)hh;
+    int rc = check_batch_args(h, q, out, query_start_loc, ctx_lens, R, T);
+    if (rc != SS_OK) return rc;
+    h->last_launches = 0;
+    if (R == 0 || T == 0) return SS_OK;
+    if (!block_table || (((uintptr_t)block_table) & 3u)) return SS_ERR_INVALID_ARG;
+    if (lse_or_null && (((uintptr_t)lse_or_null) & 3u)) return SS_ERR_INVALID_ARG;
+    if (!workspace || !aligned16(workspace)) return SS_ERR_INVALID_ARG;
+    if (workspace_bytes < h->ws.total) return SS_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    if (h->force_simple) {
+        SS_CUDA(h, launch_simple_attention(h, q, block_table, query_start_loc, ctx_lens, R, T, scale, out, lse_or_null, st),
+                "simple attention launch");
+        h->last_launches = 1;
+        return SS_OK;
+    }
+    SS_CUDA(h, launch_worklist(h, query_start_loc, ctx_lens, R, T, workspace, st), "worklist launch");
+    int n = 1;
+    SS_CUDA(h, launch_main_attention(h, q, block_table, query_start_loc, ctx_lens, R, T, scale, out, lse_or_null,
+                                     workspace, st, &n),
+            "main attention launch");
+    h->last_launches = 1 + n;
+    return SS_OK;
+}
+
+int ss_build_worklist(ss_handle* hh, const int32_t* query_start_loc, const int32_t* ctx_lens, int32_t R, int32_t T,
+                      void* workspace, size_t workspace_bytes, ss_work_item* items_host, int32_t max_items,
+                      int32_t counts_host[3], void* cuda_stream) {
+    Handle* h = (Handle*)hh;
+    if (!h || !counts_host || R < 0 || T < 0 || R > h->cfg.max_requests || T > h->cfg.max_tokens) return SS_ERR_INVALID_ARG;
+    counts_host[0] = counts_host[1] = counts_host[2] = 0;
+    if (R == 0) return SS_OK;
+    if (!query_start_loc || !ctx_lens || !workspace) return SS_ERR_INVALID_ARG;
+    if (workspace_bytes < h->ws.total) return SS_ERR_WORKSPACE_TOO_SMALL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    SS_CUDA(h, launch_worklist(h, query_start_loc, ctx_lens, R, T, workspace, st), "worklist launch");
+    WorkHeader hdr;
+    SS_CUDA(h, cudaMemcpyAsync(&hdr, (char*)workspace + h->ws.header_off, sizeof hdr, cudaMemcpyDeviceToHost, st),
+            "worklist header copy");
+    SS_CUDA(h, cudaStreamSynchronize(st), "worklist sync");
+    counts_host[0] = hdr.n_prefill;
+    counts_host[1] = hdr.n_decode;
+    counts_host[2] = hdr.n_partial;
+    if (items_host) {
+        int n = hdr.n_prefill + hdr.n_decode;
+        if (n > max_items) n = max_items;
+        if (n > 0) {
+            SS_CUDA(h, cudaMemcpyAsync(items_host, (char*)workspace + h->ws.items_off, sizeof(ss_work_item) * (size_t)n,
+                                       cudaMemcpyDeviceToHost, st),
+                    "worklist items copy");
+            SS_CUDA(h, cudaStreamSynchronize(st), "worklist sync");
+        }
+    }
+    return SS_OK;
+}
+
+int ss_iteration_host(ss_handle* hh, const void* q_host, const void* k_new_host, const void* v_new_host,
+                      const int32_t* block_table_host, const int32_t* qsl_host, const int32_t* ctx_host, int32_t R,
+                      int32_t T, float scale, void* out_host, void* cuda_stream) {
+    Handle* h = (Handle*)hh;
+    if (!h || R < 0 || T < 0 || R > h->cfg.max_requests || T > h->cfg.max_tokens) return SS_ERR_INVALID_ARG;
+    if (R == 0 || T == 0) return SS_OK;
+    if (!q_host || !block_table_host || !qsl_host || !ctx_host || !out_host) return SS_ERR_INVALID_ARG;
+    if ((k_new_host == nullptr) != (v_new_host == nullptr)) return SS_ERR_INVALID_ARG;
+    const ss_config& c = h->cfg;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t q_max = (size_t)c.max_tokens * c.num_q_heads * c.head_dim * 2;
+    const size_t kv_max = (size_t)c.max_tokens * c.num_kv_heads * c.head_dim * 2;
+    if (!h->st_q) {
+        SS_CUDA(h, cudaMalloc(&h->st_q, q_max), "staging alloc");
+        SS_CUDA(h, cudaMalloc(&h->st_out, q_max), "staging alloc");
+        SS_CUDA(h, cudaMalloc(&h->st_knew, kv_max), "staging alloc");
+        SS_CUDA(h, cudaMalloc(&h->st_vnew, kv_max), "staging alloc");
+        SS_CUDA(h, cudaMalloc(&h->st_ws, h->ws.total), "staging alloc");
+        SS_CUDA(h, cudaMalloc((void**)&h->st_bt, sizeof(int32_t) * (size_t)c.max_requests * c.max_pages_per_req), "staging alloc");
+        SS_CUDA(h, cudaMalloc((void**)&h->st_qsl, sizeof(int32_t) * (size_t)(c.max_requests + 1)), "staging alloc");
+        SS_CUDA(h, cudaMalloc((void**)&h->st_ctx, sizeof(int32_t) * (size_t)c.max_requests), "staging alloc");
+    }
+    const size_t q_bytes = (size_t)T * c.num_q_heads * c.head_dim * 2;
+    const size_t kv_bytes = (size_t)T * c.num_kv_heads * c.head_dim * 2;
+    SS_CUDA(h, cudaMemcpyAsync(h->st_q, q_host, q_bytes, cudaMemcpyHostToDevice, st), "h2d q");
+    SS_CUDA(h, cudaMemcpyAsync(h->st_bt, block_table_host, sizeof(int32_t) * (size_t)R * c.max_pages_per_req,
+                               cudaMemcpyHostToDevice, st), "h2d block_table");
+    SS_CUDA(h, cudaMemcpyAsync(h->st_qsl, qsl_host, sizeof(int32_t) * (size_t)(R + 1), cudaMemcpyHostToDevice, st), "h2d qsl");
+    SS_CUDA(h, cudaMemcpyAsync(h->st_ctx, ctx_host, sizeof(int32_t) * (size_t)R, cudaMemcpyHostToDevice, st), "h2d ctx");
+    int launches = 0;
+    if (k_new_host) {
+        SS_CUDA(h, cudaMemcpyAsync(h->st_knew, k_new_host, kv_bytes, cudaMemcpyHostToDevice, st), "h2d k_new");
+        SS_CUDA(h, cudaMemcpyAsync(h->st_vnew, v_new_host, kv_bytes, cudaMemcpyHostToDevice, st), "h2d v_new");
+        int rc = ss_kv_append(hh, h->st_knew, h->st_vnew, h->st_bt, h->st_qsl, h->st_ctx, R, T, cuda_stream);
+        if (rc != SS_OK) return rc;
+        launches += h->last_launches;
+    }
+    int rc = ss_mixed_attention(hh, h->st_q, h->st_bt, h->st_qsl, h->st_ctx, R, T, scale, h->st_out, nullptr, h->st_ws,
+                                h->ws.total, cuda_stream);
+    if (rc != SS_OK) return rc;
+    launches += h->last_launches;
+    SS_CUDA(h, cudaMemcpyAsync(out_host, h->st_out, q_bytes, cudaMemcpyDeviceToHost, st), "d2h out");
+    SS_CUDA(h, cudaStreamSynchronize(st), "iteration sync");
+    h->last_launches = launches;
+    return SS_OK;
+}
+
+}  // extern "C"

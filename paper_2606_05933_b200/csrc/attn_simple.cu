@@ -1,0 +1,164 @@
+// Plain CUDA-core attention (one warp per (query row, query head), online softmax over 32-key blocks)
+// and the split-KV merge kernel K5.
+//
+// The warp kernel is the library's in-CUDA fallback for shapes the tensor-core kernels do not cover and
+// a debugging second opinion (ss_debug_force_simple_path); it is NOT the fast path and never a CPU
+// fallback.  Same definition as everywhere: row j of request r sees keys 0..u_r+j.
+#include "common.cuh"
+
+namespace ss {
+
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+
+__device__ __forceinline__ float bf16_bits_to_float(uint32_t hi16) { return __uint_as_float(hi16 << 16); }
+
+template <int D>
+__global__ void __launch_bounds__(128)
+simple_attention_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k_cache,
+                        const __nv_bfloat16* __restrict__ v_cache, const int32_t* __restrict__ block_table,
+                        const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int T,
+                        int Hq, int Hkv, int max_pages, float scale, __nv_bfloat16* __restrict__ out,
+                        float* __restrict__ lse, int prefill_only) {
+    constexpr int EPL = D / 32;                       // output elements per lane
+    __shared__ float s_q[4][D];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t unit = (int64_t)blockIdx.x * 4 + warp;   // (row, head)
+    if (unit >= (int64_t)T * Hq) return;
+    const int row = (int)(unit / Hq), h = (int)(unit % Hq);
+    const int g = h / (Hq / Hkv);
+
+    int lo = 0, hi = R;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(qsl + mid) <= row) lo = mid; else hi = mid;
+    }
+    const int r = lo;
+    if (prefill_only && __ldg(qsl + r + 1) - __ldg(qsl + r) <= 1) return;   // decode rows are served by K4
+    const int n = __ldg(ctx_lens + r) + (row - __ldg(qsl + r)) + 1;      // visible keys
+    const int32_t* bt = block_table + (int64_t)r * max_pages;
+
+    const __nv_bfloat16* qrow = q + ((int64_t)row * Hq + h) * D;
+    for (int d = lane; d < D; d += 32) s_q[warp][d] = __bfloat162float(qrow[d]);
+    __syncwarp();
+
+    const float sl2 = scale * kLog2e;
+    float m = -INFINITY, l = 0.f, acc[EPL];
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
+
+    for (int base = 0; base < n; base += 32) {
+        const int t = base + lane;
+        const bool valid = t < n;
+        int64_t row_off = 0;
+        float s = -INFINITY;
+        if (valid) {
+            const int64_t page = __ldg(bt + (t >> 4));
+            row_off = ((page * Hkv + g) * kPage + (t & 15)) * (int64_t)D;
+            const uint4* kr = reinterpret_cast<const uint4*>(k_cache + row_off);
+            float dot = 0.f;
+#pragma unroll 4
+            for (int v = 0; v < D / 8; ++v) {
+                const uint4 w = __ldg(kr + v);
+                const float* qq = &s_q[warp][v * 8];
+                dot += qq[0] * bf16_bits_to_float(w.x & 0xffffu) + qq[1] * bf16_bits_to_float(w.x >> 16);
+                dot += qq[2] * bf16_bits_to_float(w.y & 0xffffu) + qq[3] * bf16_bits_to_float(w.y >> 16);
+                dot += qq[4] * bf16_bits_to_float(w.z & 0xffffu) + qq[5] * bf16_bits_to_float(w.z >> 16);
+                dot += qq[6] * bf16_bits_to_float(w.w & 0xffffu) + qq[7] * bf16_bits_to_float(w.w >> 16);
+            }
+            s = dot * sl2;
+        }
+        float bm = s;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) bm = fmaxf(bm, __shfl_xor_sync(0xffffffffu, bm, o));
+        const float m_new = fmaxf(m, bm);                 // finite: lane 0 of every block is valid
+        const float alpha = exp2f(m - m_new);             // exp2(-inf) = 0 on the first block
+        const float p = valid ? exp2f(s - m_new) : 0.f;
+        float ps = p;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) ps += __shfl_xor_sync(0xffffffffu, ps, o);
+        l = l * alpha + ps;
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) acc[e] *= alpha;
+        m = m_new;
+        const int cnt = min(32, n - base);
+        for (int i = 0; i < cnt; ++i) {
+            const float pi = __shfl_sync(0xffffffffu, p, i);
+            const int64_t off = __shfl_sync(0xffffffffu, row_off, i);
+            const __nv_bfloat16* vr = v_cache + off + lane * EPL;
+#pragma unroll
+            for (int e = 0; e < EPL; ++e) acc[e] += pi * __bfloat162float(vr[e]);
+        }
+    }
+    const float inv = 1.f / l;
+    __nv_bfloat16* orow = out + ((int64_t)row * Hq + h) * D + lane * EPL;
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) orow[e] = __float2bfloat16_rn(acc[e] * inv);
+    if (lse && lane == 0) lse[(int64_t)row * Hq + h] = (m + log2f(l)) * kLn2;
+}
+
+cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
+                                    const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
+                                    cudaStream_t stream, int prefill_only) {
+    const ss_config& c = h->cfg;
+    const int64_t units = (int64_t)T * c.num_q_heads;
+    const unsigned blocks = (unsigned)((units + 3) / 4);
+    if (c.head_dim == 128)
+        simple_attention_kernel<128><<<blocks, 128, 0, stream>>>(
+            (const __nv_bfloat16*)q, (const __nv_bfloat16*)h->k_cache, (const __nv_bfloat16*)h->v_cache, bt, qsl,
+            ctx, R, T, c.num_q_heads, c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
+    else
+        simple_attention_kernel<64><<<blocks, 128, 0, stream>>>(
+            (const __nv_bfloat16*)q, (const __nv_bfloat16*)h->k_cache, (const __nv_bfloat16*)h->v_cache, bt, qsl,
+            ctx, R, T, c.num_q_heads, c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// K5 split merge (a5): m = max_s m_s; l = sum_s l_s 2^(m_s - m); o = sum_s o_s 2^(m_s - m) / l, fixed
+// split order => bitwise reproducible.  Partial slot layout: [slot][G][D + 2] fp32 = o[D], m (log2
+// units), l.  One CTA per (request, kv head); warp w handles query head g*G + w of the group.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kMaxGroup * 32)
+merge_kernel(const int32_t* __restrict__ qsl, const int32_t* __restrict__ req_nsplit,
+             const int32_t* __restrict__ req_partial, const float* __restrict__ partials, int Hq, int Hkv, int D,
+             __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
+    const int r = blockIdx.x, g = blockIdx.y;
+    const int ns = req_nsplit[r];
+    if (ns <= 1) return;
+    const int G = Hq / Hkv;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (w >= G) return;
+    const int stride = D + 2;
+    const float* base = partials + ((int64_t)(req_partial[r] + g * ns) * G + w) * stride;
+    const int64_t slot_stride = (int64_t)G * stride;
+    float m = -INFINITY;
+    for (int s = 0; s < ns; ++s) m = fmaxf(m, base[s * slot_stride + D]);
+    float l = 0.f;
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};                // D <= 128 -> <= 4 elements per lane
+    for (int s = 0; s < ns; ++s) {
+        const float* p = base + s * slot_stride;
+        const float wgt = exp2f(p[D] - m);
+        l += p[D + 1] * wgt;
+        for (int e = 0, d = lane; d < D; d += 32, ++e) acc[e] += p[d] * wgt;
+    }
+    const float inv = 1.f / l;
+    const int row = qsl[r];
+    const int h = g * G + w;
+    __nv_bfloat16* orow = out + ((int64_t)row * Hq + h) * D;
+    for (int e = 0, d = lane; d < D; d += 32, ++e) orow[d] = __float2bfloat16_rn(acc[e] * inv);
+    if (lse && lane == 0) lse[(int64_t)row * Hq + h] = (m + log2f(l)) * kLn2;
+}
+
+cudaError_t launch_merge(const Handle* h, const int32_t* qsl, int R, void* workspace, void* out, float* lse,
+                         cudaStream_t stream) {
+    const ss_config& c = h->cfg;
+    char* ws = (char*)workspace;
+    dim3 grid((unsigned)R, (unsigned)c.num_kv_heads, 1);
+    merge_kernel<<<grid, h->group * 32, 0, stream>>>(
+        qsl, (const int32_t*)(ws + h->ws.req_nsplit_off), (const int32_t*)(ws + h->ws.req_partial_off),
+        (const float*)(ws + h->ws.partial_off), c.num_q_heads, c.num_kv_heads, c.head_dim, (__nv_bfloat16*)out, lse);
+    return cudaGetLastError();
+}
+
+}  // namespace ss

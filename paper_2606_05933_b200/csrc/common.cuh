@@ -1,0 +1,96 @@
+// Internal declarations shared by the translation units of libslidingattn (CUDA product path only;
+// the CPU oracle under oracle/ shares nothing with this directory).
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "slidingattn.h"
+
+namespace ss {
+
+constexpr int kPage = 16;             // tokens per KV page (BASELINE.json configs: "page 16")
+constexpr int kTileKeys = 128;        // keys per staged KV tile / MMA N
+constexpr int kTileRows = 128;        // query rows per prefill tile / MMA M
+constexpr int kMaxGroup = 16;         // max q heads per kv head on the decode path (MMA M = 16)
+constexpr int kDecodeWaves = 6;       // target decode items per SM when choosing the split length
+constexpr int kMinSplitKeys = 512;    // never split a decode KV range finer than this
+constexpr int kMaxSplitKeys = 4096;   // never leave a decode item longer than this
+
+// Workspace header written by the work-list kernel (device side, int32 words).
+struct WorkHeader {
+    int32_t n_prefill;      // prefill tile items
+    int32_t n_decode;       // decode split items
+    int32_t n_partial;      // partial slots (one per split of a split (req, kv head))
+    int32_t split_keys;     // chosen split length L (multiple of kTileKeys)
+    int32_t n_merge;        // (req, kv head) units whose splits must be merged
+    int32_t pad[11];
+};
+
+struct WorkspaceLayout {
+    size_t header_off, items_off, req_nsplit_off, req_partial_off, partial_off, total;
+    int32_t max_items, max_partials;
+};
+
+struct Handle {
+    ss_config cfg;
+    int device;
+    int num_sms;
+    int group;                       // Hq / Hkv
+    void* k_cache;
+    void* v_cache;
+    CUtensorMap tmap_k, tmap_v;      // [pages*Hkv*16 rows][D] bf16, box 16 x 64, 128B swizzle
+    bool have_tmaps;
+    WorkspaceLayout ws;
+    // host-iteration staging (lazy)
+    void *st_q, *st_knew, *st_vnew, *st_out, *st_ws;
+    int32_t *st_bt, *st_qsl, *st_ctx;
+    int last_launches;
+    int force_simple;
+    char err[256];
+};
+
+inline WorkspaceLayout workspace_layout(const ss_config& c, int num_sms) {
+    WorkspaceLayout w{};
+    const int64_t group = c.num_q_heads / c.num_kv_heads;
+    const int64_t tiles = (int64_t)(c.max_tokens + kTileRows - 1) / kTileRows + c.max_requests;
+    const int64_t max_prefill = (int64_t)c.num_q_heads * tiles;
+    // decode items: Hkv * sum_r nsplit_r.  Unclamped split length: <= Hkv*R + num_sms*kDecodeWaves;
+    // split length clamped at kMaxSplitKeys: <= Hkv * R * (ceil(max ctx / kMaxSplitKeys) + 1).
+    const int64_t max_ctx = (int64_t)c.max_pages_per_req * kPage;
+    const int64_t max_decode = (int64_t)c.num_kv_heads * c.max_requests * ((max_ctx + kMaxSplitKeys - 1) / kMaxSplitKeys + 1) +
+                               (int64_t)num_sms * kDecodeWaves + 64;
+    w.max_items = (int32_t)(max_prefill + max_decode);
+    w.max_partials = (int32_t)max_decode;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = (off + bytes + 255) & ~(size_t)255; return o; };
+    w.header_off = take(sizeof(WorkHeader));
+    w.items_off = take(sizeof(ss_work_item) * (size_t)w.max_items);
+    w.req_nsplit_off = take(sizeof(int32_t) * (size_t)(c.max_requests + 1));
+    w.req_partial_off = take(sizeof(int32_t) * (size_t)(c.max_requests + 1));
+    // partial slot = group rows of (m, l, o[D]) fp32
+    w.partial_off = take(sizeof(float) * (size_t)w.max_partials * (size_t)group * (size_t)(c.head_dim + 2));
+    w.total = off;
+    return w;
+}
+
+// ---- launchers implemented in the .cu files (all enqueue on `stream`, return cudaError_t) ----
+cudaError_t launch_kv_append(const Handle* h, const void* k_new, const void* v_new, const int32_t* bt,
+                             const int32_t* qsl, const int32_t* ctx, int R, int T, cudaStream_t stream);
+cudaError_t launch_worklist(const Handle* h, const int32_t* qsl, const int32_t* ctx, int R, int T,
+                            void* workspace, cudaStream_t stream);
+cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
+                                    const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
+                                    cudaStream_t stream, int prefill_only = 0);
+cudaError_t launch_decode(const Handle* h, const void* q, const int32_t* bt, float scale, void* workspace,
+                          void* out, float* lse, cudaStream_t stream);
+// Main path (a3 + a4 + a5): consumes the work list in `workspace`; *n_launches receives the kernel count.
+cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
+                                  const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
+                                  void* workspace, cudaStream_t stream, int* n_launches);
+cudaError_t launch_merge(const Handle* h, const int32_t* qsl, int R, void* workspace, void* out, float* lse,
+                         cudaStream_t stream);
+
+}  // namespace ss

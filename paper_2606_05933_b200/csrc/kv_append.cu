@@ -1,0 +1,49 @@
+// K1 kv_append (a1; PAPER.md:99 step 10 — request r's cached length grows by c_r).
+// One CTA per (token, K|V): the token's Hkv*D bf16 row is moved as 16-byte vectors straight into its
+// page slot.  Integer index math + bit copies only (never through a float type) => bit-exact.
+// Roofline: HBM; algorithmic bytes = 4*T*Hkv*D*2 (read + write, K and V).
+#include "common.cuh"
+
+namespace ss {
+
+__global__ void __launch_bounds__(128)
+kv_append_kernel(const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
+                 uint4* __restrict__ k_cache, uint4* __restrict__ v_cache,
+                 const int32_t* __restrict__ block_table, const int32_t* __restrict__ qsl,
+                 const int32_t* __restrict__ ctx_lens, int R, int max_pages, int Hkv, int vec_per_head) {
+    const int tok = blockIdx.x;
+    const uint4* __restrict__ src = blockIdx.y ? v_new : k_new;
+    uint4* __restrict__ dst = blockIdx.y ? v_cache : k_cache;
+
+    // request of this token: last r with qsl[r] <= tok (empty requests are skipped by construction)
+    int lo = 0, hi = R;            // invariant: qsl[lo] <= tok < qsl[hi]
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(qsl + mid) <= tok) lo = mid; else hi = mid;
+    }
+    const int r = lo;
+    const int pos = __ldg(ctx_lens + r) + (tok - __ldg(qsl + r));
+    const int64_t page = __ldg(block_table + (int64_t)r * max_pages + (pos >> 4));
+    const int slot = pos & (kPage - 1);
+
+    const int vec_per_tok = Hkv * vec_per_head;
+    const uint4* s = src + (int64_t)tok * vec_per_tok;
+    for (int v = threadIdx.x; v < vec_per_tok; v += blockDim.x) {
+        const int g = v / vec_per_head;
+        const int dv = v - g * vec_per_head;
+        const int64_t d = ((page * Hkv + g) * kPage + slot) * (int64_t)vec_per_head + dv;
+        dst[d] = __ldg(s + v);
+    }
+}
+
+cudaError_t launch_kv_append(const Handle* h, const void* k_new, const void* v_new, const int32_t* bt,
+                             const int32_t* qsl, const int32_t* ctx, int R, int T, cudaStream_t stream) {
+    const ss_config& c = h->cfg;
+    dim3 grid((unsigned)T, 2, 1);
+    kv_append_kernel<<<grid, 128, 0, stream>>>(
+        (const uint4*)k_new, (const uint4*)v_new, (uint4*)h->k_cache, (uint4*)h->v_cache, bt, qsl, ctx, R,
+        c.max_pages_per_req, c.num_kv_heads, c.head_dim / 8);
+    return cudaGetLastError();
+}
+
+}  // namespace ss
