@@ -144,6 +144,12 @@ int ss_iteration_host(ss_handle* h, const void* q_host, const void* k_new_host, 
  * caller can report launches per iteration without a profiler. */
 int ss_last_launch_count(const ss_handle* h);
 
+/* Measurement aid: when on, ss_mixed_attention brackets its dominant kernel(s) (a3+a4 main launch) with
+ * CUDA events on the caller's stream; ss_last_kernel_time_us then synchronises on them and returns the
+ * device time of the last call's main launch in microseconds (SS_ERR_INVALID_ARG if timing was off). */
+int ss_set_kernel_timing(ss_handle* h, int on);
+int ss_last_kernel_time_us(ss_handle* h, float* main_us);
+
 /* Debug: force the plain one-warp-per-row CUDA kernel (no tensor cores) for every row. 0 = off. */
 int ss_debug_force_simple_path(ss_handle* h, int on);
 

@@ -17,7 +17,8 @@ _lib = None
 SS_OK = 0
 EXPORTS = ["ss_version", "ss_status_string", "ss_last_error_string", "ss_create", "ss_destroy",
            "ss_workspace_bytes", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
-           "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path"]
+           "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path",
+           "ss_set_kernel_timing", "ss_last_kernel_time_us"]
 
 
 class ss_config(ctypes.Structure):
@@ -66,8 +67,11 @@ def load():
     lib.ss_iteration_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
     lib.ss_last_launch_count.argtypes = [vp]
     lib.ss_debug_force_simple_path.argtypes = [vp, ctypes.c_int]
+    lib.ss_set_kernel_timing.argtypes = [vp, ctypes.c_int]
+    lib.ss_last_kernel_time_us.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     for name in ("ss_create", "ss_destroy", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
-                 "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path"):
+                 "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path",
+                 "ss_set_kernel_timing", "ss_last_kernel_time_us"):
         getattr(lib, name).restype = ctypes.c_int
     _lib = lib
     return lib
@@ -163,6 +167,14 @@ class SlidingAttn:
 
     def last_launch_count(self) -> int:
         return int(self.lib.ss_last_launch_count(self._h))
+
+    def set_kernel_timing(self, on: bool):
+        self._check(self.lib.ss_set_kernel_timing(self._h, int(on)))
+
+    def last_kernel_time_us(self) -> float:
+        v = ctypes.c_float()
+        self._check(self.lib.ss_last_kernel_time_us(self._h, ctypes.byref(v)))
+        return float(v.value)
 
     def force_simple_path(self, on: bool):
         self._check(self.lib.ss_debug_force_simple_path(self._h, int(on)))

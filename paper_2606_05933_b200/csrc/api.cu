@@ -137,6 +137,8 @@ int ss_create(ss_handle** out_handle, const ss_config* cfg, void* k_cache, void*
 int ss_destroy(ss_handle* hh) {
     Handle* h = (Handle*)hh;
     if (!h) return SS_ERR_INVALID_ARG;
+    if (h->ev0) cudaEventDestroy(h->ev0);
+    if (h->ev1) cudaEventDestroy(h->ev1);
     void* bufs[] = {h->st_q, h->st_knew, h->st_vnew, h->st_out, h->st_ws, h->st_bt, h->st_qsl, h->st_ctx};
     for (void* b : bufs)
         if (b) cudaFree(b);
@@ -152,6 +154,28 @@ size_t ss_workspace_bytes(const ss_handle* hh) {
 int ss_last_launch_count(const ss_handle* hh) {
     const Handle* h = (const Handle*)hh;
     return h ? h->last_launches : 0;
+}
+
+int ss_set_kernel_timing(ss_handle* hh, int on) {
+    Handle* h = (Handle*)hh;
+    if (!h) return SS_ERR_INVALID_ARG;
+    if (on && !h->ev0) {
+        SS_CUDA(h, cudaEventCreate(&h->ev0), "event create");
+        SS_CUDA(h, cudaEventCreate(&h->ev1), "event create");
+    }
+    h->timing_on = on ? 1 : 0;
+    h->timing_valid = 0;
+    return SS_OK;
+}
+
+int ss_last_kernel_time_us(ss_handle* hh, float* main_us) {
+    Handle* h = (Handle*)hh;
+    if (!h || !main_us || !h->timing_on || !h->timing_valid) return SS_ERR_INVALID_ARG;
+    SS_CUDA(h, cudaEventSynchronize(h->ev1), "timing sync");
+    float ms = 0.f;
+    SS_CUDA(h, cudaEventElapsedTime(&ms, h->ev0, h->ev1), "timing elapsed");
+    *main_us = ms * 1000.f;
+    return SS_OK;
 }
 
 int ss_debug_force_simple_path(ss_handle* hh, int on) {
@@ -197,9 +221,14 @@ int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table,
     }
     SS_CUDA(h, launch_worklist(h, query_start_loc, ctx_lens, R, T, workspace, st), "worklist launch");
     int n = 1;
+    if (h->timing_on) SS_CUDA(h, cudaEventRecord(h->ev0, st), "timing event");
     SS_CUDA(h, launch_main_attention(h, q, block_table, query_start_loc, ctx_lens, R, T, scale, out, lse_or_null,
                                      workspace, st, &n),
             "main attention launch");
+    if (h->timing_on) {
+        SS_CUDA(h, cudaEventRecord(h->ev1, st), "timing event");
+        h->timing_valid = 1;
+    }
     h->last_launches = 1 + n;
     return SS_OK;
 }

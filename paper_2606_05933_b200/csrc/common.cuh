@@ -49,6 +49,8 @@ struct Handle {
     int32_t *st_bt, *st_qsl, *st_ctx;
     int last_launches;
     int force_simple;
+    int timing_on, timing_valid;
+    cudaEvent_t ev0, ev1;
     char err[256];
 };
 
