@@ -10,7 +10,7 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     if (e != cudaSuccess) return e;
     e = launch_merge(h, qsl, R, workspace, out, lse, stream);
     if (e != cudaSuccess) return e;
-    e = launch_simple_attention(h, q, bt, qsl, ctx, R, T, scale, out, lse, stream, /*prefill_only=*/1);
+    e = launch_prefill(h, q, bt, ctx, T, scale, workspace, out, lse, stream);
     *n_launches = 3;
     return e;
 }

@@ -86,6 +86,8 @@ cudaError_t launch_worklist(const Handle* h, const int32_t* qsl, const int32_t* 
 cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
                                     const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
                                     cudaStream_t stream, int prefill_only = 0);
+cudaError_t launch_prefill(const Handle* h, const void* q, const int32_t* bt, const int32_t* ctx, int T, float scale,
+                           void* workspace, void* out, float* lse, cudaStream_t stream);
 cudaError_t launch_decode(const Handle* h, const void* q, const int32_t* bt, float scale, void* workspace,
                           void* out, float* lse, cudaStream_t stream);
 // Main path (a3 + a4 + a5): consumes the work list in `workspace`; *n_launches receives the kernel count.

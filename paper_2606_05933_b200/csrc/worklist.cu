@@ -6,38 +6,71 @@
 //            yields ~kDecodeWaves items per SM (tile aligned, clamped to [kMinSplitKeys, kMaxSplitKeys])
 // Items of each kind are ordered heavy-first by request (longest KV range first) so the tail of the
 // persistent main kernel is short.  Integer work only; one CTA; no host read-back.
+// Phases: (A) per-request counts, (B) heavy-first ranks, (C) block scans in rank order, (D) one thread
+// per item writes its 48-byte record with three 16-byte stores.
 #include "common.cuh"
 
 namespace ss {
 
 __device__ __forceinline__ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
+// exclusive scan of a[0..n) in place (shared memory), result total returned to every thread
+__device__ int block_exclusive_scan(int32_t* a, int32_t* tmp, int n) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    // Hillis-Steele inclusive scan with ping-pong between a and tmp
+    int32_t* src = a;
+    int32_t* dst = tmp;
+    for (int off = 1; off < n; off <<= 1) {
+        for (int i = tid; i < n; i += nt) dst[i] = src[i] + (i >= off ? src[i - off] : 0);
+        __syncthreads();
+        int32_t* t = src; src = dst; dst = t;
+    }
+    const int total = n > 0 ? src[n - 1] : 0;
+    __syncthreads();
+    // shift to exclusive into `a`
+    for (int i = tid; i < n; i += nt) dst[i] = i > 0 ? src[i - 1] : 0;
+    __syncthreads();
+    if (dst != a)
+        for (int i = tid; i < n; i += nt) a[i] = dst[i];
+    __syncthreads();
+    return total;
+}
+
 __global__ void __launch_bounds__(1024)
 worklist_kernel(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int Hq, int Hkv,
                 int num_sms, WorkHeader* __restrict__ hdr, ss_work_item* __restrict__ items,
                 int32_t* __restrict__ req_nsplit, int32_t* __restrict__ req_partial, int max_items) {
     extern __shared__ int32_t sm[];
-    int32_t* s_c = sm;              // c_r
-    int32_t* s_u = s_c + R;         // u_r
-    int32_t* s_np = s_u + R;        // prefill items of r
-    int32_t* s_nd = s_np + R;       // decode items of r
-    int32_t* s_ns = s_nd + R;       // splits of r (decode)
-    int32_t* s_cost = s_ns + R;     // ordering key (KV length of the heaviest item)
+    int32_t* s_c = sm;               // c_r
+    int32_t* s_u = s_c + R;          // u_r
+    int32_t* s_ns = s_u + R;         // decode splits of r
+    int32_t* s_cost = s_ns + R;      // ordering key (KV length of the heaviest item)
+    int32_t* s_ordP = s_cost + R;    // rank k -> request (prefill)
+    int32_t* s_ordD = s_ordP + R;    // rank k -> request (decode)
+    int32_t* s_offP = s_ordD + R;    // rank k -> first prefill item
+    int32_t* s_offD = s_offP + R;    // rank k -> first decode item (relative to the decode base)
+    int32_t* s_part = s_offD + R;    // request -> partial slot base
+    int32_t* s_tmp = s_part + R;     // scan scratch
     __shared__ unsigned long long s_total_keys;
-    __shared__ int s_L;
+    __shared__ int s_L, s_nP, s_nD;
     const int tid = threadIdx.x, nt = blockDim.x;
 
-    if (tid == 0) s_total_keys = 0ull;
+    if (tid == 0) { s_total_keys = 0ull; s_nP = 0; s_nD = 0; }
     __syncthreads();
+    // ---- (A) ----
     unsigned long long my_keys = 0;
+    int my_p = 0, my_d = 0;
     for (int r = tid; r < R; r += nt) {
         const int c = qsl[r + 1] - qsl[r];
         const int u = ctx_lens[r];
         s_c[r] = c;
         s_u[r] = u;
-        if (c == 1) my_keys += (unsigned long long)(u + 1);
+        if (c == 1) { my_keys += (unsigned long long)(u + 1); ++my_d; }
+        if (c > 1) ++my_p;
     }
     if (my_keys) atomicAdd(&s_total_keys, my_keys);
+    if (my_p) atomicAdd(&s_nP, my_p);
+    if (my_d) atomicAdd(&s_nD, my_d);
     __syncthreads();
     if (tid == 0) {
         const unsigned long long units = s_total_keys * (unsigned long long)Hkv;
@@ -49,100 +82,85 @@ worklist_kernel(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx
         s_L = (int)L;
     }
     __syncthreads();
-    const int L = s_L;
+    const int L = s_L, nP = s_nP, nD = s_nD;
     for (int r = tid; r < R; r += nt) {
         const int c = s_c[r], u = s_u[r];
-        int np = 0, nd = 0, ns = 0, cost = 0;
+        int ns = 0, cost = 0;
         if (c > 1) {
-            np = ceil_div(c, kTileRows) * Hq;
             cost = u + c;
         } else if (c == 1) {
             const int n = u + 1;
-            const int ns0 = ceil_div(n, L);
-            const int chunk = ceil_div(ceil_div(n, ns0), kTileKeys) * kTileKeys;
+            const int chunk = ceil_div(ceil_div(n, ceil_div(n, L)), kTileKeys) * kTileKeys;
             ns = ceil_div(n, chunk);
-            nd = ns * Hkv;
             cost = chunk < n ? chunk : n;
         }
-        s_np[r] = np; s_nd[r] = nd; s_ns[r] = ns; s_cost[r] = cost;
+        s_ns[r] = ns;
+        s_cost[r] = cost;
     }
     __syncthreads();
-
-    // Per request: item offsets in heavy-first order (rank by cost desc, ties by index) and the
-    // partial-slot base (request order).  O(R^2 / threads) integer compares; R is a few hundred.
-    int tot_p = 0, tot_d = 0, tot_part = 0;
+    // ---- (B) heavy-first rank inside each kind; partial-slot sizes in request order ----
     for (int r = tid; r < R; r += nt) {
-        const int my_cost = s_cost[r];
-        const bool is_p = s_c[r] > 1, is_d = s_c[r] == 1;
-        int off = 0, part = 0;
-        for (int o = 0; o < R; ++o) {
-            const bool before = (s_cost[o] > my_cost) || (s_cost[o] == my_cost && o < r);
-            if (is_p && before) off += s_np[o];
-            if (is_d && before) off += s_nd[o];
-            if (o < r && s_ns[o] > 1) part += s_ns[o] * Hkv;
+        const int c = s_c[r], my_cost = s_cost[r];
+        if (c >= 1) {
+            const bool is_p = c > 1;
+            int rank = 0;
+            for (int o = 0; o < R; ++o) {
+                const int co = s_c[o];
+                const bool same = is_p ? (co > 1) : (co == 1);
+                rank += (same && (s_cost[o] > my_cost || (s_cost[o] == my_cost && o < r))) ? 1 : 0;
+            }
+            (is_p ? s_ordP : s_ordD)[rank] = r;
         }
-        const int c = s_c[r], u = s_u[r];
-        if (is_p) {
+        s_part[r] = (c == 1 && s_ns[r] > 1) ? s_ns[r] * Hkv : 0;
+    }
+    __syncthreads();
+    // ---- (C) scans ----
+    for (int k = tid; k < nP; k += nt) s_offP[k] = ceil_div(s_c[s_ordP[k]], kTileRows) * Hq;
+    for (int k = tid; k < nD; k += nt) s_offD[k] = s_ns[s_ordD[k]] * Hkv;
+    __syncthreads();
+    const int tot_p = block_exclusive_scan(s_offP, s_tmp, nP);
+    const int tot_d = block_exclusive_scan(s_offD, s_tmp, nD);
+    const int tot_part = block_exclusive_scan(s_part, s_tmp, R);
+    for (int r = tid; r < R; r += nt) {
+        const bool split = s_c[r] == 1 && s_ns[r] > 1;
+        req_nsplit[r] = s_c[r] == 1 ? s_ns[r] : 0;
+        req_partial[r] = split ? s_part[r] : -1;
+    }
+    // ---- (D) one thread per item ----
+    const int total = tot_p + tot_d;
+    for (int idx = tid; idx < total && idx < max_items; idx += nt) {
+        union { ss_work_item it; uint4 v[3]; } wu;
+        ss_work_item& it = wu.it;
+        if (idx < tot_p) {
+            int lo = 0, hi = nP;                         // last k with offP[k] <= idx
+            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (s_offP[mid] <= idx) lo = mid; else hi = mid; }
+            const int r = s_ordP[lo], local = idx - s_offP[lo];
+            const int c = s_c[r], u = s_u[r];
             const int ntile = ceil_div(c, kTileRows);
-            for (int k = 0; k < ntile; ++k) {           // heaviest (last) tile first
-                const int mt = ntile - 1 - k;
-                const int nrows = min(kTileRows, c - mt * kTileRows);
-                for (int hq = 0; hq < Hq; ++hq) {
-                    const int idx = off + k * Hq + hq;
-                    if (idx >= max_items) continue;
-                    ss_work_item it;
-                    it.kind = 1; it.req = r; it.head = hq; it.row0 = qsl[r] + mt * kTileRows; it.nrows = nrows;
-                    it.kv_begin = 0; it.kv_end = u + mt * kTileRows + nrows; it.split = 0; it.nsplit = 1;
-                    it.partial = -1; it.q_pos0 = mt * kTileRows; it.reserved = 0;
-                    items[idx] = it;                    // prefill items occupy [0, n_prefill)
-                }
-            }
+            const int mt = ntile - 1 - local / Hq;       // heaviest (last) tile first
+            const int nrows = min(kTileRows, c - mt * kTileRows);
+            it.kind = 1; it.req = r; it.head = local % Hq; it.row0 = qsl[r] + mt * kTileRows; it.nrows = nrows;
+            it.kv_begin = 0; it.kv_end = u + mt * kTileRows + nrows; it.split = 0; it.nsplit = 1;
+            it.partial = -1; it.q_pos0 = mt * kTileRows; it.reserved = 0;
+        } else {
+            const int didx = idx - tot_p;
+            int lo = 0, hi = nD;
+            while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (s_offD[mid] <= didx) lo = mid; else hi = mid; }
+            const int r = s_ordD[lo], local = didx - s_offD[lo];
+            const int n = s_u[r] + 1, ns = s_ns[r];
+            const int chunk = ceil_div(ceil_div(n, ceil_div(n, L)), kTileKeys) * kTileKeys;
+            const int s = local / Hkv, g = local % Hkv;
+            it.kind = 2; it.req = r; it.head = g; it.row0 = qsl[r]; it.nrows = 1;
+            it.kv_begin = s * chunk; it.kv_end = min(n, (s + 1) * chunk); it.split = s; it.nsplit = ns;
+            it.partial = ns > 1 ? s_part[r] + g * ns : -1; it.q_pos0 = 0; it.reserved = 0;
         }
-        req_nsplit[r] = is_d ? s_ns[r] : 0;
-        req_partial[r] = (is_d && s_ns[r] > 1) ? part : -1;
-    }
-    // totals
-    __shared__ int s_tot[3];
-    if (tid == 0) { s_tot[0] = s_tot[1] = s_tot[2] = 0; }
-    __syncthreads();
-    for (int r = tid; r < R; r += nt) {
-        tot_p += s_np[r]; tot_d += s_nd[r];
-        if (s_ns[r] > 1) tot_part += s_ns[r] * Hkv;
-    }
-    if (tot_p) atomicAdd(&s_tot[0], tot_p);
-    if (tot_d) atomicAdd(&s_tot[1], tot_d);
-    if (tot_part) atomicAdd(&s_tot[2], tot_part);
-    __syncthreads();
-    const int n_prefill = s_tot[0];
-
-    // decode items: second pass now that the prefill count (their base index) is known
-    for (int r = tid; r < R; r += nt) {
-        if (s_c[r] != 1) continue;
-        const int my_cost = s_cost[r];
-        int off = 0, part = 0;
-        for (int o = 0; o < R; ++o) {
-            const bool before = (s_cost[o] > my_cost) || (s_cost[o] == my_cost && o < r);
-            if (before) off += s_nd[o];
-            if (o < r && s_ns[o] > 1) part += s_ns[o] * Hkv;
-        }
-        const int n = s_u[r] + 1;
-        const int ns = s_ns[r];
-        const int chunk = ceil_div(ceil_div(n, ceil_div(n, L)), kTileKeys) * kTileKeys;
-        for (int s = 0; s < ns; ++s)
-            for (int g = 0; g < Hkv; ++g) {
-                const int idx = n_prefill + off + s * Hkv + g;
-                if (idx >= max_items) continue;
-                ss_work_item it;
-                it.kind = 2; it.req = r; it.head = g; it.row0 = qsl[r]; it.nrows = 1;
-                it.kv_begin = s * chunk; it.kv_end = min(n, (s + 1) * chunk); it.split = s; it.nsplit = ns;
-                it.partial = ns > 1 ? part + g * ns : -1; it.q_pos0 = 0; it.reserved = 0;
-                items[idx] = it;
-            }
+        uint4* dst = reinterpret_cast<uint4*>(items + idx);
+        dst[0] = wu.v[0]; dst[1] = wu.v[1]; dst[2] = wu.v[2];
     }
     if (tid == 0) {
-        hdr->n_prefill = s_tot[0];
-        hdr->n_decode = s_tot[1];
-        hdr->n_partial = s_tot[2];
+        hdr->n_prefill = tot_p;
+        hdr->n_decode = tot_d;
+        hdr->n_partial = tot_part;
         hdr->split_keys = L;
         hdr->n_merge = 0;
     }
@@ -153,8 +171,12 @@ cudaError_t launch_worklist(const Handle* h, const int32_t* qsl, const int32_t* 
     (void)T;
     char* ws = (char*)workspace;
     const WorkspaceLayout& w = h->ws;
-    const size_t smem = sizeof(int32_t) * 6 * (size_t)R;
-    int threads = R >= 512 ? 1024 : (R >= 128 ? 512 : 256);
+    const size_t smem = sizeof(int32_t) * 10 * (size_t)R;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(worklist_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    const int threads = 1024;
     worklist_kernel<<<1, threads, smem, stream>>>(
         qsl, ctx, R, h->cfg.num_q_heads, h->cfg.num_kv_heads, h->num_sms, (WorkHeader*)(ws + w.header_off),
         (ss_work_item*)(ws + w.items_off), (int32_t*)(ws + w.req_nsplit_off), (int32_t*)(ws + w.req_partial_off),
