@@ -1,0 +1,663 @@
+// Main kernel of the path: ONE launch serves any mix of prefill-chunk tiles (a3) and decode splits (a4) and
+// merges split partials (a5) — SURVEY.md §8(a), north_star (b)(c)(d).
+//
+// Persistent CTAs (one per SM) pull items from the device work list through a dynamic queue (atomic
+// counter), so tensor-bound prefill tiles and HBM-bound decode splits overlap across SMs and the batch
+// costs ~max(bytes/HBM, flops/tensor) instead of the sum.  6 warps per CTA:
+//   warp 0      scheduler + TMA producer.  Publishes each item to the other warps through a 4-slot smem
+//               ring, loads the Q tile (prefill) and streams 128-key K and V tiles — 8 pages x D/64 boxes of
+//               16 rows x 128 B, SWIZZLE_128B — into separate 2-slot K and V rings (K of tile t+2 can land
+//               as soon as S(t) is done, V as soon as PV(t) is done).
+//   warp 1      tcgen05.mma issuer + TMEM owner (prefill items only):
+//                 S[b] (128x128 fp32, TMEM cols 128b..) = Q K^T,  double buffered so softmax(t) overlaps S(t+1)
+//                 O    (128xD  fp32, TMEM cols 256..)  += P[b] V  (P from swizzled smem, V MN-major)
+//   warps 2..5  workers.
+//               prefill item: thread = query row (TMEM lane): tcgen05.ld S, causal/length mask by select,
+//                 online softmax (exp2, log2e folded into the scale, lazy rescale: O is only touched when a
+//                 row max grows by more than 2^8), P -> bf16 -> smem, epilogue stores rows < nrows only.
+//               decode item: warp w owns keys [32w,32w+32) of each tile: mma.sync.m16n8k16 with the G query
+//                 heads of the KV head padded to 16 rows (bandwidth-bound, wasted rows are free), online
+//                 softmax in registers with quad shuffles, cross-warp log-sum-exp merge through smem, then
+//                 either the final bf16 row or an fp32 partial; the CTA that writes the last partial of a
+//                 (request, kv head) merges all of them in fixed split order (bitwise reproducible).
+// Rooflines: decode items HBM (2*D*2 bytes per cached token per kv head), prefill items bf16 tensor
+// (4*D flop per visible (row,key) pair per head).  V rows at/after kv_end are zeroed in smem before any
+// PV product (unused slots may hold NaN; 0*NaN = NaN); masked scores are replaced, never multiplied.
+#include "common.cuh"
+#include "ptx.cuh"
+
+namespace ss {
+
+using namespace ptx;
+
+constexpr int kMixThreads = 192;
+constexpr int kNumSt = 3;            // K ring slots = V ring slots
+constexpr int kSchedSlots = 4;
+constexpr float kMLog2e = 1.4426950408889634f;
+constexpr float kMLn2 = 0.6931471805599453f;
+constexpr float kRescaleThreshold = 8.f;   // log2 units: P <= 2^8, safe in bf16 / fp32
+
+template <int D>
+struct MixSmem {
+    static constexpr int kHalves = D / 64;
+    static constexpr int kTile = kHalves * kTileKeys * 128;      // one K (or V, or Q) tile
+    static constexpr int kKOff = 0;
+    static constexpr int kVOff = kKOff + kNumSt * kTile;
+    static constexpr int kQOff = kVOff + kNumSt * kTile;         // Q tile (prefill) / cross-warp merge buffer (decode)
+    static constexpr int kMergeBytes = 4 * kMaxGroup * (D + 2) * 4;
+    static constexpr int kQBytes = ((kTile > kMergeBytes ? kTile : kMergeBytes) + 1023) / 1024 * 1024;
+    static constexpr int kBarOff = kQOff + kQBytes;
+    static constexpr int kSchedOff = kBarOff + 320;              // kSchedSlots x 48 B
+    static constexpr int kTmemSlotOff = kSchedOff + kSchedSlots * 48;
+    static constexpr int kTotal = kBarOff + 640 + 1024;
+    // TMEM columns: S0 [0,128) S1 [128,256) O [256,256+D) P0 [384,448) P1 [448,512) (P = bf16 pairs)
+    static constexpr int kTmemCols = 512;
+    static constexpr int kTmemO = 256, kTmemP = 384;
+    static_assert(kTotal <= 232448, "shared memory budget");
+};
+
+// barrier indices (8 bytes each, from kBarOff)
+enum : int {
+    B_KFULL = 0, B_VFULL = 3, B_KEMPTY_P = 6, B_KEMPTY_D = 9, B_VEMPTY_P = 12, B_VEMPTY_D = 15,
+    B_SFULL = 18, B_PFULL = 20, B_QFULL = 22, B_QEMPTY = 23, B_OFULL = 24, B_OFREE = 25, B_PVDONE = 26,
+    B_SCHED_FULL = 27, B_SCHED_EMPTY = 31, B_COUNT = 35
+};
+static_assert(B_COUNT * 8 <= 320, "barrier region");
+
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16;
+    d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32;
+    d |= (uint64_t)1 << 46;                 // descriptor version (Blackwell)
+    d |= (uint64_t)2 << 61;                 // layout type: SWIZZLE_128B
+    return d;
+}
+__host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N, int b_mn_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) |
+           ((uint32_t)(M >> 4) << 24);
+}
+
+struct MixParams {
+    const int32_t* block_table;
+    const int32_t* ctx_lens;
+    WorkHeader* hdr;
+    const ss_work_item* items;
+    int32_t* merge_counters;
+    float* partials;
+    const __nv_bfloat16* q;
+    __nv_bfloat16* out;
+    float* lse;
+    int max_pages, Hq, Hkv;
+    float scale;
+};
+
+template <int D>
+__global__ void __launch_bounds__(kMixThreads, 1)
+mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
+             const __grid_constant__ CUtensorMap tmap_v, const MixParams prm) {
+    using SM = MixSmem<D>;
+    constexpr int kHalves = SM::kHalves;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
+    const uint32_t bar0 = sbase + SM::kBarOff;
+    auto BAR = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + SM::kTmemSlotOff);
+    const ss_work_item* sched = reinterpret_cast<const ss_work_item*>(smem + SM::kSchedOff);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int Hq = prm.Hq, Hkv = prm.Hkv, G = Hq / Hkv;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kNumSt; ++s) {
+            mbar_init(BAR(B_KFULL + s), 1);
+            mbar_init(BAR(B_VFULL + s), 1);
+            mbar_init(BAR(B_KEMPTY_P + s), 1);
+            mbar_init(BAR(B_KEMPTY_D + s), 4);
+            mbar_init(BAR(B_VEMPTY_P + s), 1);
+            mbar_init(BAR(B_VEMPTY_D + s), 4);
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(BAR(B_SFULL + b), 1);
+            mbar_init(BAR(B_PFULL + b), 128);
+        }
+        mbar_init(BAR(B_QFULL), 1);
+        mbar_init(BAR(B_QEMPTY), 1);
+        mbar_init(BAR(B_OFULL), 1);
+        mbar_init(BAR(B_OFREE), 128);
+        mbar_init(BAR(B_PVDONE), 1);
+        for (int s = 0; s < kSchedSlots; ++s) {
+            mbar_init(BAR(B_SCHED_FULL + s), 1);
+            mbar_init(BAR(B_SCHED_EMPTY + s), 5);
+        }
+        fence_barrier_init();
+        prefetch_tmap(&tmap_q);
+        prefetch_tmap(&tmap_k);
+        prefetch_tmap(&tmap_v);
+    }
+    if (warp == 1) {
+        tmem_alloc(smem_u32(tmem_slot), SM::kTmemCols);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+    const uint32_t tmem_o = tmem_base + SM::kTmemO;
+    const uint32_t tmem_p = tmem_base + SM::kTmemP;
+
+    if (warp == 0) {
+        // =============================== scheduler + TMA producer ===============================
+        const int n_total = prm.hdr->n_prefill + prm.hdr->n_decode;
+        uint32_t fills[kNumSt] = {0, 0, 0};       // times slot s was filled
+        uint32_t useP[kNumSt] = {0, 0, 0}, useD[kNumSt] = {0, 0, 0};
+        int last_type[kNumSt] = {0, 0, 0};        // 1 = prefill, 2 = decode
+        uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0;
+        int prev_kind = 0;
+        for (;;) {
+            const int slot = n_sched % kSchedSlots;
+            mbar_wait(BAR(B_SCHED_EMPTY + slot), ((n_sched / kSchedSlots) & 1) ^ 1);
+            uint4* dst = reinterpret_cast<uint4*>(smem + SM::kSchedOff + slot * 48);
+            if (lane == 0) {
+                const int idx = atomicAdd(&prm.hdr->next_item, 1);
+                if (idx < n_total) {
+                    const uint4* src = reinterpret_cast<const uint4*>(prm.items + idx);
+                    dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
+                } else {
+                    dst[0] = make_uint4(0u, 0u, 0u, 0u);
+                }
+                mbar_arrive(BAR(B_SCHED_FULL + slot));
+            }
+            __syncwarp();
+            const ss_work_item w = sched[slot];
+            ++n_sched;
+            if (w.kind == 0) break;
+            const int32_t* bt = prm.block_table + (int64_t)w.req * prm.max_pages;
+            const int g = w.kind == 1 ? w.head / G : w.head;
+            if (w.kind == 1) {
+                mbar_wait(BAR(B_QEMPTY), (n_pre & 1) ^ 1);
+                if (prev_kind == 2) {
+                    // the Q region doubles as the decode merge buffer: wait until the previous (decode) item is done
+                    const uint32_t pn = n_sched - 2;
+                    mbar_wait(BAR(B_SCHED_EMPTY + pn % kSchedSlots), (pn / kSchedSlots) & 1);
+                }
+                if (lane == 0) {
+                    mbar_arrive_expect_tx(BAR(B_QFULL), (uint32_t)SM::kTile);
+#pragma unroll
+                    for (int hh = 0; hh < kHalves; ++hh)
+                        tma_load_2d(sbase + SM::kQOff + hh * (kTileRows * 128), &tmap_q, w.head * D + hh * 64, w.row0, BAR(B_QFULL));
+                }
+                ++n_pre;
+            }
+            prev_kind = w.kind;
+            for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kTileKeys, ++tile_ctr) {
+                const int s = tile_ctr % kNumSt;
+                const int npages = min(8, (w.kv_end - key0 + kPage - 1) / kPage);
+                const uint32_t bytes = (uint32_t)npages * kHalves * 2048;
+                const int p = (lane & 15) / kHalves, half = (lane & 15) % kHalves;
+                const bool issuer = (lane & 15) < 8 * kHalves && p < npages;
+                int page = 0;
+                if (issuer) page = __ldg(bt + (key0 >> 4) + p);
+                const int crow = (page * Hkv + g) * kPage;
+                const uint32_t off = half * (kTileKeys * 128) + p * (kPage * 128);
+                const uint32_t epar = last_type[s] == 1 ? ((useP[s] - 1) & 1) : ((useD[s] - 1) & 1);
+                // ---- K ----
+                if (fills[s]) mbar_wait(BAR((last_type[s] == 1 ? B_KEMPTY_P : B_KEMPTY_D) + s), epar);
+                if (lane == 0) mbar_arrive_expect_tx(BAR(B_KFULL + s), bytes);
+                __syncwarp();
+                if (lane < 16 && issuer) tma_load_2d(sbase + SM::kKOff + s * SM::kTile + off, &tmap_k, half * 64, crow, BAR(B_KFULL + s));
+                // ---- V ----
+                if (fills[s]) mbar_wait(BAR((last_type[s] == 1 ? B_VEMPTY_P : B_VEMPTY_D) + s), epar);
+                if (lane == 16) mbar_arrive_expect_tx(BAR(B_VFULL + s), bytes);
+                __syncwarp();
+                if (lane >= 16 && issuer) tma_load_2d(sbase + SM::kVOff + s * SM::kTile + off, &tmap_v, half * 64, crow, BAR(B_VFULL + s));
+                ++fills[s];
+                if (w.kind == 1) ++useP[s]; else ++useD[s];
+                last_type[s] = w.kind;
+            }
+        }
+    } else if (warp == 1) {
+        // =============================== tcgen05.mma issuer ===============================
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kTileKeys, 0);
+        constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileRows, D, 1);
+        uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_pre = 0;
+        auto issue_s = [&](uint32_t tc, uint32_t sc) {
+            const int s = tc % kNumSt, b = sc & 1;
+            mbar_wait(BAR(B_KFULL + s), (tc / kNumSt) & 1);
+            tc_fence_after();
+            if (lane == 0) {
+                const uint32_t kaddr = sbase + SM::kKOff + s * SM::kTile;
+#pragma unroll
+                for (int ks = 0; ks < D / 16; ++ks) {
+                    const uint32_t off = (ks >> 2) * (kTileRows * 128) + (ks & 3) * 32;
+                    umma_ss(tmem_base + b * 128, umma_desc_sw128(sbase + SM::kQOff + off, 16, 1024),
+                            umma_desc_sw128(kaddr + off, 16, 1024), idesc_qk, ks > 0);
+                }
+                umma_commit(BAR(B_KEMPTY_P + s));
+                umma_commit(BAR(B_SFULL + b));
+            }
+            __syncwarp();
+        };
+        for (;;) {
+            const int slot = n_sched % kSchedSlots;
+            mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
+            const ss_work_item w = sched[slot];
+            ++n_sched;
+            if (w.kind == 0) break;
+            const int ntiles = (w.kv_end - w.kv_begin + kTileKeys - 1) / kTileKeys;
+            if (w.kind == 1) {
+                mbar_wait(BAR(B_QFULL), n_pre & 1);
+                issue_s(tile_ctr, s_ctr);
+                for (int t = 0; t < ntiles; ++t) {
+                    if (t + 1 < ntiles) issue_s(tile_ctr + t + 1, s_ctr + t + 1);
+                    if (t + 1 == ntiles && lane == 0) umma_commit(BAR(B_QEMPTY));       // all S MMAs of the item issued
+                    const uint32_t sc = s_ctr + t, tc = tile_ctr + t;
+                    const int b = sc & 1, s = tc % kNumSt;
+                    mbar_wait(BAR(B_PFULL + b), (sc >> 1) & 1);
+                    if (t == 0) mbar_wait(BAR(B_OFREE), (n_pre & 1) ^ 1);               // previous epilogue drained O
+                    mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
+                    tc_fence_after();
+                    if (lane == 0) {
+                        const uint32_t vaddr = sbase + SM::kVOff + s * SM::kTile;
+#pragma unroll
+                        for (int kk = 0; kk < kTileKeys / 16; ++kk)      // A = P[b] from TMEM: 16 keys = 8 packed columns
+                            umma_ts(tmem_o, tmem_p + b * 64 + kk * 8, umma_desc_sw128(vaddr + kk * 2048, kTileKeys * 128, 1024),
+                                    idesc_pv, (t > 0 || kk > 0));
+                        umma_commit(BAR(B_VEMPTY_P + s));
+                        umma_commit(BAR(B_PVDONE));
+                        if (t == ntiles - 1) umma_commit(BAR(B_OFULL));
+                    }
+                    __syncwarp();
+                }
+                s_ctr += ntiles;
+                ++n_pre;
+            }
+            tile_ctr += ntiles;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
+        }
+    } else {
+        // =============================== workers ===============================
+        const int cw = warp - 2;                               // decode: key slice; also == TMEM lane quarter order below
+        const int quarter = warp & 3;                          // TMEM lane quarter this warp may access
+        const int row = quarter * 32 + lane;                   // prefill: query row inside the tile
+        const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
+        const int wtid = threadIdx.x - 64;                     // 0..127
+        const float sl2 = prm.scale * kMLog2e;
+        const int qrow = lane >> 2, qcol = (lane & 3) * 2;     // mma.sync fragment coordinates
+        uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_pre = 0;
+        float* merge = reinterpret_cast<float*>(smem + SM::kQOff);
+        int* flag = reinterpret_cast<int*>(smem + SM::kTmemSlotOff + 16);
+        for (;;) {
+            const int slot = n_sched % kSchedSlots;
+            mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
+            const ss_work_item w = sched[slot];
+            ++n_sched;
+            if (w.kind == 0) break;
+            const int ntiles = (w.kv_end - w.kv_begin + kTileKeys - 1) / kTileKeys;
+            if (w.kind == 1) {
+                // -------------------------- prefill tile: thread = query row --------------------------
+                const int u = __ldg(prm.ctx_lens + w.req);
+                const int limit = u + w.q_pos0 + row + 1;            // keys [0, limit) visible to this row
+                float m = -INFINITY, l = 0.f;
+                for (int t = 0; t < ntiles; ++t) {
+                    const uint32_t sc = s_ctr + t, tc = tile_ctr + t;
+                    const int b = sc & 1, s = tc % kNumSt;
+                    const int key0 = t * kTileKeys;
+                    if (key0 + kTileKeys > w.kv_end) {
+                        // zero V rows [kv_end - key0, 128): stale / unused-slot bits must not meet P = 0 in the MMA
+                        mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
+                        const uint32_t vaddr = sbase + SM::kVOff + s * SM::kTile;
+                        const int first = w.kv_end - key0;
+                        for (int i = wtid; i < (kTileKeys - first) * kHalves * 8; i += 128) {
+                            const int r = first + i / (kHalves * 8);
+                            const int c = i % (kHalves * 8);
+                            const uint32_t a = vaddr + (c >> 3) * (kTileKeys * 128) + r * 128 + (c & 7) * 16;
+                            asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+                        }
+                    }
+                    mbar_wait(BAR(B_SFULL + b), (sc >> 1) & 1);
+                    tc_fence_after();
+                    uint32_t sr[4][32];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) tmem_ld_32x32b_x32(tmem_base + b * 128 + lane_addr + c * 32, sr[c]);
+                    tmem_ld_wait();
+                    const int nvis = limit - key0;
+                    float bm = -INFINITY;
+                    if (nvis >= kTileKeys) {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c)
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) bm = fmaxf(bm, __uint_as_float(sr[c][i]));
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c)
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) {
+                                if (c * 32 + i >= nvis) sr[c][i] = 0xff800000u;   // -inf by select, never by arithmetic
+                                bm = fmaxf(bm, __uint_as_float(sr[c][i]));
+                            }
+                    }
+                    // lazy rescale: only move the reference max when it grows by more than 2^8
+                    const float cand = bm * sl2;
+                    float m_new = m, alpha = 1.f;
+                    if (cand > m + kRescaleThreshold) { m_new = cand; alpha = exp2f(m - m_new); }   // tile 0: m = -inf -> alpha = 0
+                    float psum = 0.f;
+                    // P = exp2(s*sl2 - m_new) -> bf16 pairs -> TMEM (A operand of the PV MMA), 64 packed columns per row
+#pragma unroll
+                    for (int hh = 0; hh < 2; ++hh) {
+                        uint32_t pk[32];
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) {
+                            const float p0 = exp2f(__uint_as_float(sr[2 * hh + (i >> 4)][(2 * i) & 31]) * sl2 - m_new);
+                            const float p1 = exp2f(__uint_as_float(sr[2 * hh + (i >> 4)][((2 * i) & 31) + 1]) * sl2 - m_new);
+                            psum += p0 + p1;
+                            pk[i] = pack_bf16(p0, p1);
+                        }
+                        tmem_st_32x32b_x32(tmem_p + b * 64 + lane_addr + hh * 32, pk);
+                    }
+                    l = l * alpha + psum;
+                    m = m_new;
+                    if (t > 0 && !__all_sync(0xffffffffu, alpha == 1.f)) {
+                        mbar_wait(BAR(B_PVDONE), (sc - 1) & 1);          // PV(t-1) must have landed in O
+                        tc_fence_after();
+#pragma unroll
+                        for (int c = 0; c < D / 32; ++c) {
+                            uint32_t orr[32];
+                            tmem_ld_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
+                            tmem_ld_wait();
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) orr[i] = __float_as_uint(__uint_as_float(orr[i]) * alpha);
+                            tmem_st_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
+                        }
+                    }
+                    tmem_st_wait();
+                    tc_fence_before();
+                    if (key0 + kTileKeys > w.kv_end) fence_proxy_async();   // zeroed V rows -> visible to the MMA's async proxy
+                    mbar_arrive(BAR(B_PFULL + b));
+                }
+                // ---- epilogue ----
+                mbar_wait(BAR(B_OFULL), n_pre & 1);
+                tc_fence_after();
+                const float inv = 1.f / l;
+                const bool store = row < w.nrows;
+                __nv_bfloat16* orow = prm.out + ((int64_t)(w.row0 + row) * Hq + w.head) * D;
+#pragma unroll
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t orr[32];
+                    tmem_ld_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
+                    tmem_ld_wait();
+                    if (store) {
+#pragma unroll
+                        for (int v = 0; v < 4; ++v) {
+                            uint4 pk;
+                            pk.x = pack_bf16(__uint_as_float(orr[v * 8 + 0]) * inv, __uint_as_float(orr[v * 8 + 1]) * inv);
+                            pk.y = pack_bf16(__uint_as_float(orr[v * 8 + 2]) * inv, __uint_as_float(orr[v * 8 + 3]) * inv);
+                            pk.z = pack_bf16(__uint_as_float(orr[v * 8 + 4]) * inv, __uint_as_float(orr[v * 8 + 5]) * inv);
+                            pk.w = pack_bf16(__uint_as_float(orr[v * 8 + 6]) * inv, __uint_as_float(orr[v * 8 + 7]) * inv);
+                            *reinterpret_cast<uint4*>(orow + c * 32 + v * 8) = pk;
+                        }
+                    }
+                }
+                if (store && prm.lse) prm.lse[(int64_t)(w.row0 + row) * Hq + w.head] = (m + log2f(l)) * kMLn2;
+                tc_fence_before();
+                mbar_arrive(BAR(B_OFREE));
+                s_ctr += ntiles;
+                ++n_pre;
+            } else {
+                // -------------------------- decode split: warp = 32-key slice --------------------------
+                uint32_t qa[D / 16][4];
+                {
+                    const __nv_bfloat16* qb = prm.q + ((int64_t)w.row0 * Hq + (int64_t)w.head * G) * D;
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        const int d0 = ks * 16 + qcol;
+                        qa[ks][0] = qrow < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)qrow * D + d0) : 0u;
+                        qa[ks][1] = qrow + 8 < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)(qrow + 8) * D + d0) : 0u;
+                        qa[ks][2] = qrow < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)qrow * D + d0 + 8) : 0u;
+                        qa[ks][3] = qrow + 8 < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)(qrow + 8) * D + d0 + 8) : 0u;
+                    }
+                }
+                float o[D / 8][4];
+#pragma unroll
+                for (int i = 0; i < D / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+                float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+                for (int t = 0; t < ntiles; ++t) {
+                    const uint32_t tc = tile_ctr + t;
+                    const int s = tc % kNumSt;
+                    const uint32_t fpar = (tc / kNumSt) & 1;
+                    const int key0 = w.kv_begin + t * kTileKeys;
+                    const int nvalid = w.kv_end - (key0 + 32 * cw);
+                    const uint32_t kbase = sbase + SM::kKOff + s * SM::kTile;
+                    const uint32_t vbase = sbase + SM::kVOff + s * SM::kTile;
+                    float sacc[4][4];
+                    mbar_wait(BAR(B_KFULL + s), fpar);
+                    if (nvalid > 0) {
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt) sacc[nt][0] = sacc[nt][1] = sacc[nt][2] = sacc[nt][3] = 0.f;
+#pragma unroll
+                        for (int j = 0; j < D / 32; ++j) {
+#pragma unroll
+                            for (int nt = 0; nt < 4; ++nt) {
+                                const int r = 32 * cw + nt * 8 + (lane & 7);
+                                const int cd = 4 * j + (lane >> 3);
+                                const uint32_t a = kbase + (cd >> 3) * (kTileKeys * 128) + r * 128 + (((cd & 7) ^ (r & 7)) << 4);
+                                uint32_t b0, b1, b2, b3;
+                                ldmatrix_x4(b0, b1, b2, b3, a);
+                                mma_bf16_16816(sacc[nt], qa[2 * j], b0, b1);
+                                mma_bf16_16816(sacc[nt], qa[2 * j + 1], b2, b3);
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(BAR(B_KEMPTY_D + s));
+                    mbar_wait(BAR(B_VFULL + s), fpar);
+                    if (nvalid > 0) {
+                        if (nvalid < 32) {
+                            for (int i = lane; i < (32 - nvalid) * kHalves * 8; i += 32) {
+                                const int r = 32 * cw + nvalid + i / (kHalves * 8);
+                                const int c = i % (kHalves * 8);
+                                const uint32_t a = vbase + (c >> 3) * (kTileKeys * 128) + r * 128 + (c & 7) * 16;
+                                asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+                            }
+                            __syncwarp();
+                        }
+                        float bm0 = -INFINITY, bm1 = -INFINITY;
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt) {
+                            const int c = nt * 8 + qcol;
+                            if (c >= nvalid) { sacc[nt][0] = -INFINITY; sacc[nt][2] = -INFINITY; }
+                            if (c + 1 >= nvalid) { sacc[nt][1] = -INFINITY; sacc[nt][3] = -INFINITY; }
+                            bm0 = fmaxf(bm0, fmaxf(sacc[nt][0], sacc[nt][1]));
+                            bm1 = fmaxf(bm1, fmaxf(sacc[nt][2], sacc[nt][3]));
+                        }
+                        bm0 = fmaxf(bm0, __shfl_xor_sync(0xffffffffu, bm0, 1));
+                        bm0 = fmaxf(bm0, __shfl_xor_sync(0xffffffffu, bm0, 2));
+                        bm1 = fmaxf(bm1, __shfl_xor_sync(0xffffffffu, bm1, 1));
+                        bm1 = fmaxf(bm1, __shfl_xor_sync(0xffffffffu, bm1, 2));
+                        const float mn0 = fmaxf(m0, bm0 * sl2), mn1 = fmaxf(m1, bm1 * sl2);
+                        const float al0 = exp2f(m0 - mn0), al1 = exp2f(m1 - mn1);
+                        float ps0 = 0.f, ps1 = 0.f;
+                        uint32_t pa[2][4];
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt) {
+                            const float p0 = exp2f(sacc[nt][0] * sl2 - mn0), p1 = exp2f(sacc[nt][1] * sl2 - mn0);
+                            const float p2 = exp2f(sacc[nt][2] * sl2 - mn1), p3 = exp2f(sacc[nt][3] * sl2 - mn1);
+                            ps0 += p0 + p1;
+                            ps1 += p2 + p3;
+                            pa[nt >> 1][(nt & 1) * 2 + 0] = pack_bf16(p0, p1);
+                            pa[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2, p3);
+                        }
+                        l0 = l0 * al0 + ps0;
+                        l1 = l1 * al1 + ps1;
+                        m0 = mn0;
+                        m1 = mn1;
+#pragma unroll
+                        for (int i = 0; i < D / 8; ++i) { o[i][0] *= al0; o[i][1] *= al0; o[i][2] *= al1; o[i][3] *= al1; }
+#pragma unroll
+                        for (int kk = 0; kk < 2; ++kk) {
+#pragma unroll
+                            for (int np = 0; np < D / 16; ++np) {
+                                const int r = 32 * cw + kk * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
+                                const int cd = 2 * np + (lane >> 4);
+                                const uint32_t a = vbase + (cd >> 3) * (kTileKeys * 128) + r * 128 + (((cd & 7) ^ (r & 7)) << 4);
+                                uint32_t b0, b1, b2, b3;
+                                ldmatrix_x4_trans(b0, b1, b2, b3, a);
+                                mma_bf16_16816(o[2 * np], pa[kk], b0, b1);
+                                mma_bf16_16816(o[2 * np + 1], pa[kk], b2, b3);
+                            }
+                        }
+                        if (nvalid < 32) fence_proxy_async();
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(BAR(B_VEMPTY_D + s));
+                }
+                // ---- cross-warp log-sum-exp merge through smem ----
+                l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
+                l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+                l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
+                l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+                float* mine = merge + cw * kMaxGroup * (D + 2);
+#pragma unroll
+                for (int i = 0; i < D / 8; ++i) {
+                    *reinterpret_cast<float2*>(mine + qrow * (D + 2) + i * 8 + qcol) = make_float2(o[i][0], o[i][1]);
+                    *reinterpret_cast<float2*>(mine + (qrow + 8) * (D + 2) + i * 8 + qcol) = make_float2(o[i][2], o[i][3]);
+                }
+                if ((lane & 3) == 0) {
+                    mine[qrow * (D + 2) + D] = m0;
+                    mine[qrow * (D + 2) + D + 1] = l0;
+                    mine[(qrow + 8) * (D + 2) + D] = m1;
+                    mine[(qrow + 8) * (D + 2) + D + 1] = l1;
+                }
+                named_bar_sync(1, 128);
+                for (int e = wtid; e < G * D; e += 128) {
+                    const int r = e / D, d = e % D;
+                    float M = -INFINITY;
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) M = fmaxf(M, merge[(x * kMaxGroup + r) * (D + 2) + D]);
+                    float L = 0.f, acc = 0.f;
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) {
+                        const float* src = merge + (x * kMaxGroup + r) * (D + 2);
+                        const float wgt = exp2f(src[D] - M);
+                        L += src[D + 1] * wgt;
+                        acc += src[d] * wgt;
+                    }
+                    if (w.nsplit == 1) {
+                        const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r;
+                        prm.out[orow * D + d] = __float2bfloat16_rn(acc / L);
+                        if (prm.lse && d == 0) prm.lse[orow] = (M + log2f(L)) * kMLn2;
+                    } else {
+                        float* dst = prm.partials + ((int64_t)(w.partial + w.split) * G + r) * (D + 2);
+                        dst[d] = acc;
+                        if (d == 0) { dst[D] = M; dst[D + 1] = L; }
+                    }
+                }
+                if (w.nsplit > 1) {
+                    // ---- a5: the CTA that completes the last split of (req, kv head) merges all splits ----
+                    __threadfence();
+                    named_bar_sync(1, 128);
+                    if (wtid == 0) {
+                        const int old = atomicAdd(prm.merge_counters + w.req * Hkv + w.head, 1);
+                        *flag = (old == w.nsplit - 1);
+                    }
+                    named_bar_sync(1, 128);
+                    if (*flag) {
+                        __threadfence();
+                        for (int e = wtid; e < G * D; e += 128) {
+                            const int r = e / D, d = e % D;
+                            const float* base = prm.partials + ((int64_t)w.partial * G + r) * (D + 2);
+                            const int64_t sstride = (int64_t)G * (D + 2);
+                            float M = -INFINITY;
+                            for (int x = 0; x < w.nsplit; ++x) M = fmaxf(M, __ldcg(base + x * sstride + D));
+                            float L = 0.f, acc = 0.f;
+                            for (int x = 0; x < w.nsplit; ++x) {
+                                const float wgt = exp2f(__ldcg(base + x * sstride + D) - M);
+                                L += __ldcg(base + x * sstride + D + 1) * wgt;
+                                acc += __ldcg(base + x * sstride + d) * wgt;
+                            }
+                            const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r;
+                            prm.out[orow * D + d] = __float2bfloat16_rn(acc / L);
+                            if (prm.lse && d == 0) prm.lse[orow] = (M + log2f(L)) * kMLn2;
+                        }
+                    }
+                }
+                named_bar_sync(1, 128);
+            }
+            tile_ctr += ntiles;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
+        }
+    }
+
+    // ---- teardown ----
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem_base, SM::kTmemCols);
+}
+
+// Per-call Q tensor map: q viewed as [T rows][Hq*D] bf16, box = 128 rows x 64 columns, 128B swizzle.
+static bool encode_q_map(CUtensorMap* map, const void* q, int T, int Hq, int D) {
+    typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                      const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) != cudaSuccess ||
+            qres != cudaDriverEntryPointSuccess)
+            return false;
+        fn = (EncodeTiledFn)p;
+    }
+    cuuint64_t gdim[2] = {(cuuint64_t)Hq * D, (cuuint64_t)T};
+    cuuint64_t gstride[1] = {(cuuint64_t)Hq * D * 2};
+    cuuint32_t box[2] = {64u, (cuuint32_t)kTileRows};
+    cuuint32_t estr[2] = {1u, 1u};
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(q), gdim, gstride, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
+                                  const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
+                                  void* workspace, cudaStream_t stream, int* n_launches) {
+    (void)qsl; (void)R;
+    const ss_config& c = h->cfg;
+    char* ws = (char*)workspace;
+    CUtensorMap tmap_q;
+    if (!encode_q_map(&tmap_q, q, T, c.num_q_heads, c.head_dim)) return cudaErrorInvalidValue;
+    MixParams p;
+    p.block_table = bt;
+    p.ctx_lens = ctx;
+    p.hdr = (WorkHeader*)(ws + h->ws.header_off);
+    p.items = (const ss_work_item*)(ws + h->ws.items_off);
+    p.merge_counters = (int32_t*)(ws + h->ws.counters_off);
+    p.partials = (float*)(ws + h->ws.partial_off);
+    p.q = (const __nv_bfloat16*)q;
+    p.out = (__nv_bfloat16*)out;
+    p.lse = lse;
+    p.max_pages = c.max_pages_per_req;
+    p.Hq = c.num_q_heads;
+    p.Hkv = c.num_kv_heads;
+    p.scale = scale;
+    *n_launches = 1;
+    cudaError_t e;
+    if (c.head_dim == 128) {
+        auto kern = mixed_kernel<128>;
+        constexpr int smem = MixSmem<128>::kTotal;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        kern<<<h->num_sms, kMixThreads, smem, stream>>>(tmap_q, h->tmap_k, h->tmap_v, p);
+    } else {
+        auto kern = mixed_kernel<64>;
+        constexpr int smem = MixSmem<64>::kTotal;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        kern<<<h->num_sms, kMixThreads, smem, stream>>>(tmap_q, h->tmap_k, h->tmap_v, p);
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace ss

@@ -1,5 +1,4 @@
-// Plain CUDA-core attention (one warp per (query row, query head), online softmax over 32-key blocks)
-// and the split-KV merge kernel K5.
+// Plain CUDA-core attention (one warp per (query row, query head), online softmax over 32-key blocks).
 //
 // The warp kernel is the library's in-CUDA fallback for shapes the tensor-core kernels do not cover and
 // a debugging second opinion (ss_debug_force_simple_path); it is NOT the fast path and never a CPU
@@ -111,53 +110,6 @@ cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_
         simple_attention_kernel<64><<<blocks, 128, 0, stream>>>(
             (const __nv_bfloat16*)q, (const __nv_bfloat16*)h->k_cache, (const __nv_bfloat16*)h->v_cache, bt, qsl,
             ctx, R, T, c.num_q_heads, c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
-    return cudaGetLastError();
-}
-
-// ------------------------------------------------------------------------------------------------
-// K5 split merge (a5): m = max_s m_s; l = sum_s l_s 2^(m_s - m); o = sum_s o_s 2^(m_s - m) / l, fixed
-// split order => bitwise reproducible.  Partial slot layout: [slot][G][D + 2] fp32 = o[D], m (log2
-// units), l.  One CTA per (request, kv head); warp w handles query head g*G + w of the group.
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kMaxGroup * 32)
-merge_kernel(const int32_t* __restrict__ qsl, const int32_t* __restrict__ req_nsplit,
-             const int32_t* __restrict__ req_partial, const float* __restrict__ partials, int Hq, int Hkv, int D,
-             __nv_bfloat16* __restrict__ out, float* __restrict__ lse) {
-    const int r = blockIdx.x, g = blockIdx.y;
-    const int ns = req_nsplit[r];
-    if (ns <= 1) return;
-    const int G = Hq / Hkv;
-    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (w >= G) return;
-    const int stride = D + 2;
-    const float* base = partials + ((int64_t)(req_partial[r] + g * ns) * G + w) * stride;
-    const int64_t slot_stride = (int64_t)G * stride;
-    float m = -INFINITY;
-    for (int s = 0; s < ns; ++s) m = fmaxf(m, base[s * slot_stride + D]);
-    float l = 0.f;
-    float acc[4] = {0.f, 0.f, 0.f, 0.f};                // D <= 128 -> <= 4 elements per lane
-    for (int s = 0; s < ns; ++s) {
-        const float* p = base + s * slot_stride;
-        const float wgt = exp2f(p[D] - m);
-        l += p[D + 1] * wgt;
-        for (int e = 0, d = lane; d < D; d += 32, ++e) acc[e] += p[d] * wgt;
-    }
-    const float inv = 1.f / l;
-    const int row = qsl[r];
-    const int h = g * G + w;
-    __nv_bfloat16* orow = out + ((int64_t)row * Hq + h) * D;
-    for (int e = 0, d = lane; d < D; d += 32, ++e) orow[d] = __float2bfloat16_rn(acc[e] * inv);
-    if (lse && lane == 0) lse[(int64_t)row * Hq + h] = (m + log2f(l)) * kLn2;
-}
-
-cudaError_t launch_merge(const Handle* h, const int32_t* qsl, int R, void* workspace, void* out, float* lse,
-                         cudaStream_t stream) {
-    const ss_config& c = h->cfg;
-    char* ws = (char*)workspace;
-    dim3 grid((unsigned)R, (unsigned)c.num_kv_heads, 1);
-    merge_kernel<<<grid, h->group * 32, 0, stream>>>(
-        qsl, (const int32_t*)(ws + h->ws.req_nsplit_off), (const int32_t*)(ws + h->ws.req_partial_off),
-        (const float*)(ws + h->ws.partial_off), c.num_q_heads, c.num_kv_heads, c.head_dim, (__nv_bfloat16*)out, lse);
     return cudaGetLastError();
 }
 

@@ -25,12 +25,12 @@ struct WorkHeader {
     int32_t n_decode;       // decode split items
     int32_t n_partial;      // partial slots (one per split of a split (req, kv head))
     int32_t split_keys;     // chosen split length L (multiple of kTileKeys)
-    int32_t n_merge;        // (req, kv head) units whose splits must be merged
+    int32_t next_item;      // dynamic queue head of the main kernel (zeroed by the work-list kernel)
     int32_t pad[11];
 };
 
 struct WorkspaceLayout {
-    size_t header_off, items_off, req_nsplit_off, req_partial_off, partial_off, total;
+    size_t header_off, items_off, counters_off, partial_off, total;
     int32_t max_items, max_partials;
 };
 
@@ -70,8 +70,7 @@ inline WorkspaceLayout workspace_layout(const ss_config& c, int num_sms) {
     auto take = [&](size_t bytes) { size_t o = off; off = (off + bytes + 255) & ~(size_t)255; return o; };
     w.header_off = take(sizeof(WorkHeader));
     w.items_off = take(sizeof(ss_work_item) * (size_t)w.max_items);
-    w.req_nsplit_off = take(sizeof(int32_t) * (size_t)(c.max_requests + 1));
-    w.req_partial_off = take(sizeof(int32_t) * (size_t)(c.max_requests + 1));
+    w.counters_off = take(sizeof(int32_t) * (size_t)c.max_requests * (size_t)c.num_kv_heads);   // split arrival counters
     // partial slot = group rows of (m, l, o[D]) fp32
     w.partial_off = take(sizeof(float) * (size_t)w.max_partials * (size_t)group * (size_t)(c.head_dim + 2));
     w.total = off;
@@ -86,15 +85,9 @@ cudaError_t launch_worklist(const Handle* h, const int32_t* qsl, const int32_t* 
 cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
                                     const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
                                     cudaStream_t stream, int prefill_only = 0);
-cudaError_t launch_prefill(const Handle* h, const void* q, const int32_t* bt, const int32_t* ctx, int T, float scale,
-                           void* workspace, void* out, float* lse, cudaStream_t stream);
-cudaError_t launch_decode(const Handle* h, const void* q, const int32_t* bt, float scale, void* workspace,
-                          void* out, float* lse, cudaStream_t stream);
 // Main path (a3 + a4 + a5): consumes the work list in `workspace`; *n_launches receives the kernel count.
 cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
                                   const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
                                   void* workspace, cudaStream_t stream, int* n_launches);
-cudaError_t launch_merge(const Handle* h, const int32_t* qsl, int R, void* workspace, void* out, float* lse,
-                         cudaStream_t stream);
 
 }  // namespace ss

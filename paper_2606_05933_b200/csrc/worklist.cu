@@ -39,7 +39,7 @@ __device__ int block_exclusive_scan(int32_t* a, int32_t* tmp, int n) {
 __global__ void __launch_bounds__(1024)
 worklist_kernel(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int Hq, int Hkv,
                 int num_sms, WorkHeader* __restrict__ hdr, ss_work_item* __restrict__ items,
-                int32_t* __restrict__ req_nsplit, int32_t* __restrict__ req_partial, int max_items) {
+                int32_t* __restrict__ merge_counters, int max_items) {
     extern __shared__ int32_t sm[];
     int32_t* s_c = sm;               // c_r
     int32_t* s_u = s_c + R;          // u_r
@@ -121,11 +121,7 @@ worklist_kernel(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx
     const int tot_p = block_exclusive_scan(s_offP, s_tmp, nP);
     const int tot_d = block_exclusive_scan(s_offD, s_tmp, nD);
     const int tot_part = block_exclusive_scan(s_part, s_tmp, R);
-    for (int r = tid; r < R; r += nt) {
-        const bool split = s_c[r] == 1 && s_ns[r] > 1;
-        req_nsplit[r] = s_c[r] == 1 ? s_ns[r] : 0;
-        req_partial[r] = split ? s_part[r] : -1;
-    }
+    for (int i = tid; i < R * Hkv; i += nt) merge_counters[i] = 0;     // "last split merges" arrival counters
     // ---- (D) one thread per item ----
     const int total = tot_p + tot_d;
     for (int idx = tid; idx < total && idx < max_items; idx += nt) {
@@ -162,7 +158,7 @@ worklist_kernel(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx
         hdr->n_decode = tot_d;
         hdr->n_partial = tot_part;
         hdr->split_keys = L;
-        hdr->n_merge = 0;
+        hdr->next_item = 0;
     }
 }
 
@@ -179,8 +175,7 @@ cudaError_t launch_worklist(const Handle* h, const int32_t* qsl, const int32_t* 
     const int threads = 1024;
     worklist_kernel<<<1, threads, smem, stream>>>(
         qsl, ctx, R, h->cfg.num_q_heads, h->cfg.num_kv_heads, h->num_sms, (WorkHeader*)(ws + w.header_off),
-        (ss_work_item*)(ws + w.items_off), (int32_t*)(ws + w.req_nsplit_off), (int32_t*)(ws + w.req_partial_off),
-        w.max_items);
+        (ss_work_item*)(ws + w.items_off), (int32_t*)(ws + w.counters_off), w.max_items);
     return cudaGetLastError();
 }
 
