@@ -43,6 +43,8 @@ def get_batch(name: str):
         return wl.config_c5()
     if name.startswith("PP-"):
         return wl.config_scene_edge(name)
+    if name.startswith("PD-"):
+        return wl.config_decode_only(name)
     if name.startswith("C3:"):
         C, n, nd = (int(x) for x in name[3:].split(","))
         return wl.config_c3(C, n, nd)

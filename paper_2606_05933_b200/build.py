@@ -40,7 +40,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed building libslidingattn.so")
-    (PKG / "build_ptxas.log").write_text(res.stdout + res.stderr)
+    log = "\n".join(l for l in (res.stdout + res.stderr).splitlines() if "Compile time" not in l)
+    (PKG / "build_ptxas.log").write_text(log + "\n")
     os.replace(tmp, LIB)
     return LIB
 

@@ -178,6 +178,21 @@ def config_scene_edge(name: str) -> Batch:
     return make_batch(name, Hq, Hkv, 128, reqs, seed)
 
 
+def config_decode_only(name: str) -> Batch:
+    """PD-* scene edges: the decode set of a named mixed config alone (C = 0).
+    PD-C2 / PD-C5: the decodes of C2 / C5; PD-32 / PD-128: the C3 decode sets (median 1500)."""
+    if name == "PD-C2":
+        src = config_c2()
+    elif name == "PD-C5":
+        src = config_c5()
+    elif name in ("PD-32", "PD-128"):
+        return config_c3(0, 1, int(name[3:]))
+    else:
+        raise KeyError(name)
+    reqs = [(c, u) for c, u in src.reqs if c == 1]
+    return make_batch(name, src.num_q_heads, src.num_kv_heads, src.head_dim, reqs, 7100 + len(reqs))
+
+
 def random_batch(seed: int, Hq: int = 8, Hkv: int = 2, D: int = 128, n_prefill: int = 2,
                  n_decode: int = 5, max_c: int = 200, max_u: int = 600, n_empty: int = 1,
                  with_append: bool = True) -> Batch:
