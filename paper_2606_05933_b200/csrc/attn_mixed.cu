@@ -149,133 +149,143 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
 
     if (warp == 0) {
         // =============================== scheduler + TMA producer ===============================
-        const int n_total = prm.hdr->n_prefill + prm.hdr->n_decode;
-        uint32_t fills[kNumSt] = {0, 0, 0};       // times slot s was filled
-        uint32_t useP[kNumSt] = {0, 0, 0}, useD[kNumSt] = {0, 0, 0};
-        int last_type[kNumSt] = {0, 0, 0};        // 1 = prefill, 2 = decode
-        uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0;
-        int prev_kind = 0;
-        for (;;) {
-            const int slot = n_sched % kSchedSlots;
-            mbar_wait(BAR(B_SCHED_EMPTY + slot), ((n_sched / kSchedSlots) & 1) ^ 1);
-            uint4* dst = reinterpret_cast<uint4*>(smem + SM::kSchedOff + slot * 48);
-            if (lane == 0) {
+        // One elected thread runs the whole loop (waits included) so every TMA operand is uniform.
+        if (elect_one()) {
+            const int n_total = prm.hdr->n_prefill + prm.hdr->n_decode;
+            // per-slot history as bit fields: parity of the next EMPTY wait per consumer type, last consumer type
+            uint32_t parP = 0, parD = 0, lastT = 0;
+            uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0;
+            int prev_kind = 0;
+            for (;;) {
+                const int slot = n_sched % kSchedSlots;
+                mbar_wait(BAR(B_SCHED_EMPTY + slot), ((n_sched / kSchedSlots) & 1) ^ 1);
+                uint4* dst = reinterpret_cast<uint4*>(smem + SM::kSchedOff + slot * 48);
+                union { ss_work_item it; uint4 v[3]; } wu;
                 const int idx = atomicAdd(&prm.hdr->next_item, 1);
                 if (idx < n_total) {
                     const uint4* src = reinterpret_cast<const uint4*>(prm.items + idx);
-                    dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
+                    wu.v[0] = __ldg(src); wu.v[1] = __ldg(src + 1); wu.v[2] = __ldg(src + 2);
                 } else {
-                    dst[0] = make_uint4(0u, 0u, 0u, 0u);
+                    wu.v[0] = wu.v[1] = wu.v[2] = make_uint4(0u, 0u, 0u, 0u);
                 }
-                mbar_arrive(BAR(B_SCHED_FULL + slot));
-            }
-            __syncwarp();
-            const ss_work_item w = sched[slot];
-            ++n_sched;
-            if (w.kind == 0) break;
-            const int32_t* bt = prm.block_table + (int64_t)w.req * prm.max_pages;
-            const int g = w.kind == 1 ? w.head / G : w.head;
-            if (w.kind == 1) {
-                mbar_wait(BAR(B_QEMPTY), (n_pre & 1) ^ 1);
-                if (prev_kind == 2) {
-                    // the Q region doubles as the decode merge buffer: wait until the previous (decode) item is done
-                    const uint32_t pn = n_sched - 2;
-                    mbar_wait(BAR(B_SCHED_EMPTY + pn % kSchedSlots), (pn / kSchedSlots) & 1);
-                }
-                if (lane == 0) {
+                dst[0] = wu.v[0]; dst[1] = wu.v[1]; dst[2] = wu.v[2];
+                mbar_arrive(BAR(B_SCHED_FULL + slot));        // release semantics: the item is visible to the waiters
+                const ss_work_item& w = wu.it;
+                ++n_sched;
+                if (w.kind == 0) break;
+                const int32_t* bt = prm.block_table + (int64_t)w.req * prm.max_pages;
+                const int g = w.kind == 1 ? w.head / G : w.head;
+                int pg[8];
+                auto load_pages = [&](int key0) {
+#pragma unroll
+                    for (int p = 0; p < 8; ++p) pg[p] = (key0 + p * kPage < w.kv_end) ? __ldg(bt + (key0 >> 4) + p) : 0;
+                };
+                load_pages(w.kv_begin);
+                if (w.kind == 1) {
+                    mbar_wait(BAR(B_QEMPTY), (n_pre & 1) ^ 1);
+                    if (prev_kind == 2) {
+                        // the Q region doubles as the decode merge buffer: wait until the previous (decode) item is done
+                        const uint32_t pn = n_sched - 2;
+                        mbar_wait(BAR(B_SCHED_EMPTY + pn % kSchedSlots), (pn / kSchedSlots) & 1);
+                    }
                     mbar_arrive_expect_tx(BAR(B_QFULL), (uint32_t)SM::kTile);
 #pragma unroll
                     for (int hh = 0; hh < kHalves; ++hh)
                         tma_load_2d(sbase + SM::kQOff + hh * (kTileRows * 128), &tmap_q, w.head * D + hh * 64, w.row0, BAR(B_QFULL));
+                    ++n_pre;
                 }
-                ++n_pre;
-            }
-            prev_kind = w.kind;
-            for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kTileKeys, ++tile_ctr) {
-                const int s = tile_ctr % kNumSt;
-                const int npages = min(8, (w.kv_end - key0 + kPage - 1) / kPage);
-                const uint32_t bytes = (uint32_t)npages * kHalves * 2048;
-                const int p = (lane & 15) / kHalves, half = (lane & 15) % kHalves;
-                const bool issuer = (lane & 15) < 8 * kHalves && p < npages;
-                int page = 0;
-                if (issuer) page = __ldg(bt + (key0 >> 4) + p);
-                const int crow = (page * Hkv + g) * kPage;
-                const uint32_t off = half * (kTileKeys * 128) + p * (kPage * 128);
-                const uint32_t epar = last_type[s] == 1 ? ((useP[s] - 1) & 1) : ((useD[s] - 1) & 1);
-                // ---- K ----
-                if (fills[s]) mbar_wait(BAR((last_type[s] == 1 ? B_KEMPTY_P : B_KEMPTY_D) + s), epar);
-                if (lane == 0) mbar_arrive_expect_tx(BAR(B_KFULL + s), bytes);
-                __syncwarp();
-                if (lane < 16 && issuer) tma_load_2d(sbase + SM::kKOff + s * SM::kTile + off, &tmap_k, half * 64, crow, BAR(B_KFULL + s));
-                // ---- V ----
-                if (fills[s]) mbar_wait(BAR((last_type[s] == 1 ? B_VEMPTY_P : B_VEMPTY_D) + s), epar);
-                if (lane == 16) mbar_arrive_expect_tx(BAR(B_VFULL + s), bytes);
-                __syncwarp();
-                if (lane >= 16 && issuer) tma_load_2d(sbase + SM::kVOff + s * SM::kTile + off, &tmap_v, half * 64, crow, BAR(B_VFULL + s));
-                ++fills[s];
-                if (w.kind == 1) ++useP[s]; else ++useD[s];
-                last_type[s] = w.kind;
+                prev_kind = w.kind;
+                for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kTileKeys, ++tile_ctr) {
+                    const int s = tile_ctr % kNumSt;
+                    const int npages = min(8, (w.kv_end - key0 + kPage - 1) / kPage);
+                    const uint32_t bytes = (uint32_t)npages * kHalves * 2048;
+                    int crow[8];
+#pragma unroll
+                    for (int p = 0; p < 8; ++p) crow[p] = (pg[p] * Hkv + g) * kPage;
+                    if (key0 + kTileKeys < w.kv_end) load_pages(key0 + kTileKeys);      // next tile's page ids in flight
+                    const uint32_t lt = (lastT >> (2 * s)) & 3u;
+                    const uint32_t epar = ((lt == 1 ? parP : parD) >> s) & 1u;
+                    // ---- K ----
+                    if (lt) mbar_wait(BAR((lt == 1 ? B_KEMPTY_P : B_KEMPTY_D) + s), epar);
+                    mbar_arrive_expect_tx(BAR(B_KFULL + s), bytes);
+#pragma unroll
+                    for (int p = 0; p < 8; ++p)
+                        if (p < npages) {
+#pragma unroll
+                            for (int hh = 0; hh < kHalves; ++hh)
+                                tma_load_2d(sbase + SM::kKOff + s * SM::kTile + hh * (kTileKeys * 128) + p * (kPage * 128),
+                                            &tmap_k, hh * 64, crow[p], BAR(B_KFULL + s));
+                        }
+                    // ---- V ----
+                    if (lt) mbar_wait(BAR((lt == 1 ? B_VEMPTY_P : B_VEMPTY_D) + s), epar);
+                    mbar_arrive_expect_tx(BAR(B_VFULL + s), bytes);
+#pragma unroll
+                    for (int p = 0; p < 8; ++p)
+                        if (p < npages) {
+#pragma unroll
+                            for (int hh = 0; hh < kHalves; ++hh)
+                                tma_load_2d(sbase + SM::kVOff + s * SM::kTile + hh * (kTileKeys * 128) + p * (kPage * 128),
+                                            &tmap_v, hh * 64, crow[p], BAR(B_VFULL + s));
+                        }
+                    if (lt == 1) parP ^= 1u << s; else if (lt == 2) parD ^= 1u << s;
+                    lastT = (lastT & ~(3u << (2 * s))) | ((uint32_t)w.kind << (2 * s));
+                }
             }
         }
     } else if (warp == 1) {
         // =============================== tcgen05.mma issuer ===============================
-        constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kTileKeys, 0);
-        constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileRows, D, 1);
-        uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_pre = 0;
-        auto issue_s = [&](uint32_t tc, uint32_t sc) {
-            const int s = tc % kNumSt, b = sc & 1;
-            mbar_wait(BAR(B_KFULL + s), (tc / kNumSt) & 1);
-            tc_fence_after();
-            if (lane == 0) {
-                const uint32_t kaddr = sbase + SM::kKOff + s * SM::kTile;
+        // One elected thread runs the whole loop (waits included): descriptors stay in uniform registers.
+        if (elect_one()) {
+            constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kTileKeys, 0);
+            constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileRows, D, 1);
+            const uint64_t qdesc0 = umma_desc_sw128(sbase + SM::kQOff, 16, 1024);
+            uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_pre = 0;
+            auto issue_s = [&](uint32_t tc, uint32_t sc) {
+                const int s = tc % kNumSt, b = sc & 1;
+                mbar_wait(BAR(B_KFULL + s), (tc / kNumSt) & 1);
+                tc_fence_after();
+                const uint64_t kdesc0 = umma_desc_sw128(sbase + SM::kKOff + s * SM::kTile, 16, 1024);
 #pragma unroll
                 for (int ks = 0; ks < D / 16; ++ks) {
-                    const uint32_t off = (ks >> 2) * (kTileRows * 128) + (ks & 3) * 32;
-                    umma_ss(tmem_base + b * 128, umma_desc_sw128(sbase + SM::kQOff + off, 16, 1024),
-                            umma_desc_sw128(kaddr + off, 16, 1024), idesc_qk, ks > 0);
+                    const uint32_t off = (ks >> 2) * (kTileRows * 128) + (ks & 3) * 32;      // bytes; descriptor address unit = 16 B
+                    umma_ss(tmem_base + b * 128, qdesc0 + (off >> 4), kdesc0 + (off >> 4), idesc_qk, ks > 0);
                 }
                 umma_commit(BAR(B_KEMPTY_P + s));
                 umma_commit(BAR(B_SFULL + b));
-            }
-            __syncwarp();
-        };
-        for (;;) {
-            const int slot = n_sched % kSchedSlots;
-            mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
-            const ss_work_item w = sched[slot];
-            ++n_sched;
-            if (w.kind == 0) break;
-            const int ntiles = (w.kv_end - w.kv_begin + kTileKeys - 1) / kTileKeys;
-            if (w.kind == 1) {
-                mbar_wait(BAR(B_QFULL), n_pre & 1);
-                issue_s(tile_ctr, s_ctr);
-                for (int t = 0; t < ntiles; ++t) {
-                    if (t + 1 < ntiles) issue_s(tile_ctr + t + 1, s_ctr + t + 1);
-                    if (t + 1 == ntiles && lane == 0) umma_commit(BAR(B_QEMPTY));       // all S MMAs of the item issued
-                    const uint32_t sc = s_ctr + t, tc = tile_ctr + t;
-                    const int b = sc & 1, s = tc % kNumSt;
-                    mbar_wait(BAR(B_PFULL + b), (sc >> 1) & 1);
-                    if (t == 0) mbar_wait(BAR(B_OFREE), (n_pre & 1) ^ 1);               // previous epilogue drained O
-                    mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
-                    tc_fence_after();
-                    if (lane == 0) {
-                        const uint32_t vaddr = sbase + SM::kVOff + s * SM::kTile;
+            };
+            for (;;) {
+                const int slot = n_sched % kSchedSlots;
+                mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
+                const int kind = sched[slot].kind;
+                const int ntiles = (sched[slot].kv_end - sched[slot].kv_begin + kTileKeys - 1) / kTileKeys;
+                ++n_sched;
+                if (kind == 0) break;
+                if (kind == 1) {
+                    mbar_wait(BAR(B_QFULL), n_pre & 1);
+                    issue_s(tile_ctr, s_ctr);
+                    for (int t = 0; t < ntiles; ++t) {
+                        if (t + 1 < ntiles) issue_s(tile_ctr + t + 1, s_ctr + t + 1);
+                        if (t + 1 == ntiles) umma_commit(BAR(B_QEMPTY));                    // all S MMAs of the item issued
+                        const uint32_t sc = s_ctr + t, tc = tile_ctr + t;
+                        const int b = sc & 1, s = tc % kNumSt;
+                        mbar_wait(BAR(B_PFULL + b), (sc >> 1) & 1);
+                        if (t == 0) mbar_wait(BAR(B_OFREE), (n_pre & 1) ^ 1);               // previous epilogue drained O
+                        mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
+                        tc_fence_after();
+                        const uint64_t vdesc0 = umma_desc_sw128(sbase + SM::kVOff + s * SM::kTile, kTileKeys * 128, 1024);
 #pragma unroll
                         for (int kk = 0; kk < kTileKeys / 16; ++kk)      // A = P[b] from TMEM: 16 keys = 8 packed columns
-                            umma_ts(tmem_o, tmem_p + b * 64 + kk * 8, umma_desc_sw128(vaddr + kk * 2048, kTileKeys * 128, 1024),
-                                    idesc_pv, (t > 0 || kk > 0));
+                            umma_ts(tmem_o, tmem_p + b * 64 + kk * 8, vdesc0 + (uint64_t)(kk * 2048 >> 4), idesc_pv, (t > 0 || kk > 0));
                         umma_commit(BAR(B_VEMPTY_P + s));
                         umma_commit(BAR(B_PVDONE));
                         if (t == ntiles - 1) umma_commit(BAR(B_OFULL));
                     }
-                    __syncwarp();
+                    s_ctr += ntiles;
+                    ++n_pre;
                 }
-                s_ctr += ntiles;
-                ++n_pre;
+                tile_ctr += ntiles;
+                mbar_arrive(BAR(B_SCHED_EMPTY + slot));
             }
-            tile_ctr += ntiles;
-            __syncwarp();
-            if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
         }
     } else {
         // =============================== workers ===============================
@@ -594,7 +604,10 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     // ---- teardown ----
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) tmem_dealloc(tmem_base, SM::kTmemCols);
+    if (warp == 1) {
+        __syncwarp();
+        tmem_dealloc(tmem_base, SM::kTmemCols);
+    }
 }
 
 // Per-call Q tensor map: q viewed as [T rows][Hq*D] bf16, box = 128 rows x 64 columns, 128B swizzle.
