@@ -153,6 +153,12 @@ int ss_last_kernel_time_us(ss_handle* h, float* main_us);
 /* Debug: force the plain one-warp-per-row CUDA kernel (no tensor cores) for every row. 0 = off. */
 int ss_debug_force_simple_path(ss_handle* h, int on);
 
+/* Debug / tuning knobs; value 0 restores the automatic choice.  which: 1 = CTAs of the main launch (default one
+ * per SM), 2 = number of CTAs that drain the decode queue first (default: balanced from the batch's decode bytes and
+ * prefill flops by the work-list kernel; -1 = none), 3 = decode split length in keys (multiple of 128).
+ * Results never depend on these; only timing does.  SS_ERR_INVALID_ARG for an unknown key. */
+int ss_debug_set_param(ss_handle* h, int which, int value);
+
 const char* ss_status_string(int status);
 const char* ss_last_error_string(const ss_handle* h);   /* detail of the last SS_ERR_CUDA on this handle */
 int ss_version(void);

@@ -18,7 +18,7 @@ SS_OK = 0
 EXPORTS = ["ss_version", "ss_status_string", "ss_last_error_string", "ss_create", "ss_destroy",
            "ss_workspace_bytes", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
            "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path",
-           "ss_set_kernel_timing", "ss_last_kernel_time_us"]
+           "ss_debug_set_param", "ss_set_kernel_timing", "ss_last_kernel_time_us"]
 
 
 class ss_config(ctypes.Structure):
@@ -67,11 +67,12 @@ def load():
     lib.ss_iteration_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
     lib.ss_last_launch_count.argtypes = [vp]
     lib.ss_debug_force_simple_path.argtypes = [vp, ctypes.c_int]
+    lib.ss_debug_set_param.argtypes = [vp, ctypes.c_int, ctypes.c_int]
     lib.ss_set_kernel_timing.argtypes = [vp, ctypes.c_int]
     lib.ss_last_kernel_time_us.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     for name in ("ss_create", "ss_destroy", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
                  "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path",
-                 "ss_set_kernel_timing", "ss_last_kernel_time_us"):
+                 "ss_debug_set_param", "ss_set_kernel_timing", "ss_last_kernel_time_us"):
         getattr(lib, name).restype = ctypes.c_int
     _lib = lib
     return lib
@@ -178,6 +179,10 @@ class SlidingAttn:
 
     def force_simple_path(self, on: bool):
         self._check(self.lib.ss_debug_force_simple_path(self._h, int(on)))
+
+    def debug_set_param(self, which: int, value: int):
+        """1 = main-launch CTAs, 2 = decode-first CTAs, 3 = decode split keys; 0 = automatic."""
+        self._check(self.lib.ss_debug_set_param(self._h, int(which), int(value)))
 
 
 def kv_append(handle: SlidingAttn, k_new, v_new, block_table, query_start_loc, ctx_lens, stream=None):

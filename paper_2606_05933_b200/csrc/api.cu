@@ -185,6 +185,13 @@ int ss_debug_force_simple_path(ss_handle* hh, int on) {
     return SS_OK;
 }
 
+int ss_debug_set_param(ss_handle* hh, int which, int value) {
+    Handle* h = (Handle*)hh;
+    if (!h || which < 1 || which >= 8) return SS_ERR_INVALID_ARG;
+    h->dbg[which] = value;
+    return SS_OK;
+}
+
 int ss_kv_append(ss_handle* hh, const void* k_new, const void* v_new, const int32_t* block_table,
                  const int32_t* query_start_loc, const int32_t* ctx_lens, int32_t R, int32_t T, void* cuda_stream) {
     Handle* h = (Handle*)hh;

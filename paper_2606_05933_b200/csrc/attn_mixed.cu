@@ -143,6 +143,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
+    pdl_wait();                 // everything above overlaps the tail of the work-list kernel
     const uint32_t tmem_base = *tmem_slot;
     const uint32_t tmem_o = tmem_base + SM::kTmemO;
     const uint32_t tmem_p = tmem_base + SM::kTmemP;
@@ -151,7 +152,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         // =============================== scheduler + TMA producer ===============================
         // One elected thread runs the whole loop (waits included) so every TMA operand is uniform.
         if (elect_one()) {
-            const int n_total = prm.hdr->n_prefill + prm.hdr->n_decode;
+            const int n_pre_items = prm.hdr->n_prefill, n_dec = prm.hdr->n_decode;
+            const bool prefer_decode = (int)blockIdx.x < prm.hdr->n_decode_ctas;
+            bool pre_done = n_pre_items == 0, dec_done = n_dec == 0;
             // per-slot history as bit fields: parity of the next EMPTY wait per consumer type, last consumer type
             uint32_t parP = 0, parD = 0, lastT = 0;
             uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0;
@@ -161,8 +164,16 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 mbar_wait(BAR(B_SCHED_EMPTY + slot), ((n_sched / kSchedSlots) & 1) ^ 1);
                 uint4* dst = reinterpret_cast<uint4*>(smem + SM::kSchedOff + slot * 48);
                 union { ss_work_item it; uint4 v[3]; } wu;
-                const int idx = atomicAdd(&prm.hdr->next_item, 1);
-                if (idx < n_total) {
+                // two typed queues: this CTA drains its preferred kind first, then helps with the other
+                int idx = -1;
+                if (prefer_decode) {
+                    if (!dec_done) { const int i = atomicAdd(&prm.hdr->next_decode, 1); if (i < n_dec) idx = n_pre_items + i; else dec_done = true; }
+                    if (idx < 0 && !pre_done) { const int i = atomicAdd(&prm.hdr->next_prefill, 1); if (i < n_pre_items) idx = i; else pre_done = true; }
+                } else {
+                    if (!pre_done) { const int i = atomicAdd(&prm.hdr->next_prefill, 1); if (i < n_pre_items) idx = i; else pre_done = true; }
+                    if (idx < 0 && !dec_done) { const int i = atomicAdd(&prm.hdr->next_decode, 1); if (i < n_dec) idx = n_pre_items + i; else dec_done = true; }
+                }
+                if (idx >= 0) {
                     const uint4* src = reinterpret_cast<const uint4*>(prm.items + idx);
                     wu.v[0] = __ldg(src); wu.v[1] = __ldg(src + 1); wu.v[2] = __ldg(src + 2);
                 } else {
@@ -656,19 +667,22 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     p.Hkv = c.num_kv_heads;
     p.scale = scale;
     *n_launches = 1;
+    const int grid = h->dbg[kDbgGrid] > 0 ? h->dbg[kDbgGrid] : h->num_sms;
     cudaError_t e;
     if (c.head_dim == 128) {
         auto kern = mixed_kernel<128>;
         constexpr int smem = MixSmem<128>::kTotal;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        kern<<<h->num_sms, kMixThreads, smem, stream>>>(tmap_q, h->tmap_k, h->tmap_v, p);
+        e = launch_pdl(kern, dim3(grid), dim3(kMixThreads), smem, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+        if (e != cudaSuccess) return e;
     } else {
         auto kern = mixed_kernel<64>;
         constexpr int smem = MixSmem<64>::kTotal;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        kern<<<h->num_sms, kMixThreads, smem, stream>>>(tmap_q, h->tmap_k, h->tmap_v, p);
+        e = launch_pdl(kern, dim3(grid), dim3(kMixThreads), smem, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+        if (e != cudaSuccess) return e;
     }
     return cudaGetLastError();
 }

@@ -18,6 +18,13 @@ constexpr int kMaxGroup = 16;         // max q heads per kv head on the decode p
 constexpr int kDecodeWaves = 6;       // target decode items per SM when choosing the split length
 constexpr int kMinSplitKeys = 512;    // never split a decode KV range finer than this
 constexpr int kMaxSplitKeys = 4096;   // never leave a decode item longer than this
+// SM partition model of the two-queue scheduler (measured on B200): bytes/us one SM streams on the
+// decode path, flop/us one SM sustains on the prefill path, and the CTA count past which decode is HBM-limited.
+constexpr float kDecodeBytesPerUsPerSm = 80e3f;
+constexpr float kPrefillFlopsPerUsPerSm = 6.0e6f;
+constexpr int kMaxDecodeCtas = 88;
+// ss_debug_set_param keys (tuning / measurement aids; 0 restores the automatic choice)
+enum { kDbgGrid = 1, kDbgDecodeCtas = 2, kDbgSplitKeys = 3 };
 
 // Workspace header written by the work-list kernel (device side, int32 words).
 struct WorkHeader {
@@ -25,8 +32,10 @@ struct WorkHeader {
     int32_t n_decode;       // decode split items
     int32_t n_partial;      // partial slots (one per split of a split (req, kv head))
     int32_t split_keys;     // chosen split length L (multiple of kTileKeys)
-    int32_t next_item;      // dynamic queue head of the main kernel (zeroed by the work-list kernel)
-    int32_t pad[11];
+    int32_t next_prefill;   // dynamic queue heads of the main kernel (zeroed by the work-list kernel)
+    int32_t next_decode;
+    int32_t n_decode_ctas;  // CTAs [0, n_decode_ctas) drain the decode queue first, the others the prefill queue first
+    int32_t pad[9];
 };
 
 struct WorkspaceLayout {
@@ -49,6 +58,7 @@ struct Handle {
     int32_t *st_bt, *st_qsl, *st_ctx;
     int last_launches;
     int force_simple;
+    int dbg[8];                      // ss_debug_set_param knobs (0 = automatic)
     int timing_on, timing_valid;
     cudaEvent_t ev0, ev1;
     char err[256];
@@ -75,6 +85,23 @@ inline WorkspaceLayout workspace_layout(const ss_config& c, int num_sms) {
     w.partial_off = take(sizeof(float) * (size_t)w.max_partials * (size_t)group * (size_t)(c.head_dim + 2));
     w.total = off;
     return w;
+}
+
+// Launch with programmatic stream serialization: the grid may start while its predecessor in the stream drains;
+// every kernel launched this way executes griddepcontrol.wait before it touches global memory.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
 // ---- launchers implemented in the .cu files (all enqueue on `stream`, return cudaError_t) ----

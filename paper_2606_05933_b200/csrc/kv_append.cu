@@ -3,6 +3,7 @@
 // page slot.  Integer index math + bit copies only (never through a float type) => bit-exact.
 // Roofline: HBM; algorithmic bytes = 4*T*Hkv*D*2 (read + write, K and V).
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace ss {
 
@@ -11,6 +12,8 @@ kv_append_kernel(const uint4* __restrict__ k_new, const uint4* __restrict__ v_ne
                  uint4* __restrict__ k_cache, uint4* __restrict__ v_cache,
                  const int32_t* __restrict__ block_table, const int32_t* __restrict__ qsl,
                  const int32_t* __restrict__ ctx_lens, int R, int max_pages, int Hkv, int vec_per_head) {
+    ptx::pdl_launch_dependents();
+    ptx::pdl_wait();
     const int tok = blockIdx.x;
     const uint4* __restrict__ src = blockIdx.y ? v_new : k_new;
     uint4* __restrict__ dst = blockIdx.y ? v_cache : k_cache;
@@ -40,10 +43,9 @@ cudaError_t launch_kv_append(const Handle* h, const void* k_new, const void* v_n
                              const int32_t* qsl, const int32_t* ctx, int R, int T, cudaStream_t stream) {
     const ss_config& c = h->cfg;
     dim3 grid((unsigned)T, 2, 1);
-    kv_append_kernel<<<grid, 128, 0, stream>>>(
-        (const uint4*)k_new, (const uint4*)v_new, (uint4*)h->k_cache, (uint4*)h->v_cache, bt, qsl, ctx, R,
-        c.max_pages_per_req, c.num_kv_heads, c.head_dim / 8);
-    return cudaGetLastError();
+    return launch_pdl(kv_append_kernel, grid, dim3(128), 0, stream, (const uint4*)k_new, (const uint4*)v_new,
+                      (uint4*)h->k_cache, (uint4*)h->v_cache, bt, qsl, ctx, R, c.max_pages_per_req, c.num_kv_heads,
+                      c.head_dim / 8);
 }
 
 }  // namespace ss
