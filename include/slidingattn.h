@@ -159,6 +159,12 @@ int ss_debug_force_simple_path(ss_handle* h, int on);
  * Results never depend on these; only timing does.  SS_ERR_INVALID_ARG for an unknown key. */
 int ss_debug_set_param(ss_handle* h, int which, int value);
 
+/* Measurement aid: per-CTA timeline of the main launch.  `trace_dev` is a DEVICE buffer of
+ * num_ctas * words_per_cta uint64 words (caller-owned; NULL switches tracing off).  Per CTA the kernel writes
+ * word 0 = %globaltimer at entry (ns), 1 = after setup + grid dependency wait, 2 = at exit, 3 = item count, then
+ * 3 words per item (start ns, end ns, kind << 32 | KV tiles) while they fit.  Results never depend on it. */
+int ss_debug_set_trace(ss_handle* h, void* trace_dev, int32_t words_per_cta);
+
 const char* ss_status_string(int status);
 const char* ss_last_error_string(const ss_handle* h);   /* detail of the last SS_ERR_CUDA on this handle */
 int ss_version(void);

@@ -18,7 +18,7 @@ SS_OK = 0
 EXPORTS = ["ss_version", "ss_status_string", "ss_last_error_string", "ss_create", "ss_destroy",
            "ss_workspace_bytes", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
            "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path",
-           "ss_debug_set_param", "ss_set_kernel_timing", "ss_last_kernel_time_us"]
+           "ss_debug_set_param", "ss_debug_set_trace", "ss_set_kernel_timing", "ss_last_kernel_time_us"]
 
 
 class ss_config(ctypes.Structure):
@@ -68,11 +68,12 @@ def load():
     lib.ss_last_launch_count.argtypes = [vp]
     lib.ss_debug_force_simple_path.argtypes = [vp, ctypes.c_int]
     lib.ss_debug_set_param.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+    lib.ss_debug_set_trace.argtypes = [vp, vp, i32]
     lib.ss_set_kernel_timing.argtypes = [vp, ctypes.c_int]
     lib.ss_last_kernel_time_us.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     for name in ("ss_create", "ss_destroy", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
                  "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path",
-                 "ss_debug_set_param", "ss_set_kernel_timing", "ss_last_kernel_time_us"):
+                 "ss_debug_set_param", "ss_debug_set_trace", "ss_set_kernel_timing", "ss_last_kernel_time_us"):
         getattr(lib, name).restype = ctypes.c_int
     _lib = lib
     return lib
@@ -183,6 +184,12 @@ class SlidingAttn:
     def debug_set_param(self, which: int, value: int):
         """1 = main-launch CTAs, 2 = decode-first CTAs, 3 = decode split keys; 0 = automatic."""
         self._check(self.lib.ss_debug_set_param(self._h, int(which), int(value)))
+
+
+    def set_trace(self, buf: Optional[torch.Tensor], words_per_cta: int = 0):
+        """Per-CTA timeline of the main launch into a CUDA int64 tensor [num_ctas, words_per_cta]; None = off."""
+        self._trace_buf = buf
+        self._check(self.lib.ss_debug_set_trace(self._h, _ptr(buf), int(words_per_cta)))
 
 
 def kv_append(handle: SlidingAttn, k_new, v_new, block_table, query_start_loc, ctx_lens, stream=None):

@@ -192,6 +192,14 @@ int ss_debug_set_param(ss_handle* hh, int which, int value) {
     return SS_OK;
 }
 
+int ss_debug_set_trace(ss_handle* hh, void* trace_dev, int32_t words_per_cta) {
+    Handle* h = (Handle*)hh;
+    if (!h || (trace_dev && words_per_cta < 4) || (((uintptr_t)trace_dev) & 7u)) return SS_ERR_INVALID_ARG;
+    h->trace = (unsigned long long*)trace_dev;
+    h->trace_words = trace_dev ? words_per_cta : 0;
+    return SS_OK;
+}
+
 int ss_kv_append(ss_handle* hh, const void* k_new, const void* v_new, const int32_t* block_table,
                  const int32_t* query_start_loc, const int32_t* ctx_lens, int32_t R, int32_t T, void* cuda_stream) {
     Handle* h = (Handle*)hh;

@@ -90,6 +90,8 @@ struct MixParams {
     float* lse;
     int max_pages, Hq, Hkv;
     float scale;
+    unsigned long long* trace;     // ss_debug_set_trace: per-CTA timeline, or null
+    int trace_words;
 };
 
 template <int D>
@@ -108,6 +110,8 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int Hq = prm.Hq, Hkv = prm.Hkv, G = Hq / Hkv;
+    unsigned long long* const trace = prm.trace ? prm.trace + (size_t)blockIdx.x * prm.trace_words : nullptr;
+    if (trace && threadIdx.x == 0) trace[0] = globaltimer_ns();
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < kNumSt; ++s) {
@@ -144,6 +148,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     __syncthreads();
     tc_fence_after();
     pdl_wait();                 // everything above overlaps the tail of the work-list kernel
+    if (trace && threadIdx.x == 0) trace[1] = globaltimer_ns();
     const uint32_t tmem_base = *tmem_slot;
     const uint32_t tmem_o = tmem_base + SM::kTmemO;
     const uint32_t tmem_p = tmem_base + SM::kTmemP;
@@ -317,6 +322,10 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             ++n_sched;
             if (w.kind == 0) break;
             const int ntiles = (w.kv_end - w.kv_begin + kTileKeys - 1) / kTileKeys;
+            if (trace && wtid == 0 && 4 + 3 * (int)n_sched <= prm.trace_words) {
+                trace[4 + 3 * (n_sched - 1)] = globaltimer_ns();
+                trace[4 + 3 * (n_sched - 1) + 2] = ((unsigned long long)w.kind << 32) | (unsigned)ntiles;
+            }
             if (w.kind == 1) {
                 // -------------------------- prefill tile: thread = query row --------------------------
                 const int u = __ldg(prm.ctx_lens + w.req);
@@ -607,9 +616,11 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 named_bar_sync(1, 128);
             }
             tile_ctr += ntiles;
+            if (trace && wtid == 0 && 4 + 3 * (int)n_sched <= prm.trace_words) trace[4 + 3 * (n_sched - 1) + 1] = globaltimer_ns();
             __syncwarp();
             if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
         }
+        if (trace && wtid == 0) { trace[2] = globaltimer_ns(); trace[3] = n_sched - 1; }
     }
 
     // ---- teardown ----
@@ -666,6 +677,8 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     p.Hq = c.num_q_heads;
     p.Hkv = c.num_kv_heads;
     p.scale = scale;
+    p.trace = h->trace;
+    p.trace_words = h->trace_words;
     *n_launches = 1;
     const int grid = h->dbg[kDbgGrid] > 0 ? h->dbg[kDbgGrid] : h->num_sms;
     cudaError_t e;

@@ -59,6 +59,8 @@ struct Handle {
     int last_launches;
     int force_simple;
     int dbg[8];                      // ss_debug_set_param knobs (0 = automatic)
+    unsigned long long* trace;       // ss_debug_set_trace buffer (device) or null
+    int trace_words;
     int timing_on, timing_valid;
     cudaEvent_t ev0, ev1;
     char err[256];

@@ -1,0 +1,138 @@
+"""Measured latency surface of one mixed_attention iteration over chunk-token budget x decode count x
+context length (north_star): what a SlidingChunker-style batch latency predictor
+(§3.2, Eq. 4-5, Table 1) would be fitted on.
+
+    python -m paper_2606_05933_b200.surface --out gpurun_out/surface.csv [--with-c4]
+
+One CSV row per point: config id, seed, R, T, x1..x7 (Table 1), algorithmic bytes and flops, t_HBM, t_TC,
+roofline, measured us (median, p10, p90 over >= 30 timed iterations after >= 5 warm-ups, CUDA events on the
+launching stream, L2 flushed between iterations outside the event window), fraction of the batch
+roofline, and for mixed points overlap = t_mixed / (t_prefill_only + t_decode_only).
+
+Needs a B200 and the built library (no CPU fallback).  Imports nothing from oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import csv
+import sys
+from pathlib import Path
+from typing import List, Optional
+
+import numpy as np
+
+from . import accounting as acc
+from . import workloads as wl
+from .features import features, scene
+
+FIELDS = ["point", "name", "seed", "shape", "scene", "R", "T", "chunk", "n_prefill", "n_decode", "ctx_median",
+          "x1", "x2", "x3", "x4", "x5", "x6", "x7", "bytes", "flops", "t_hbm_us", "t_tc_us", "roofline_us", "bound",
+          "median_us", "p10_us", "p90_us", "frac_of_roofline", "prefill_only_us", "decode_only_us", "overlap"]
+
+
+def surface_points(with_c4: bool = False) -> List[tuple]:
+    """(point id, Batch factory) for the whole grid, in a fixed order."""
+    pts = []
+    for nd in (32, 128):                                   # BASELINE.json configs[2]: the predictor grid
+        for C in (256, 512, 1024, 2048):
+            for n in (1, 2, 3, 4):
+                pts.append((f"C3:{C},{n},{nd}", lambda C=C, n=n, nd=nd: wl.config_c3(C, n, nd)))
+    for med in (500, 4000):                                # third axis: decode-context length
+        for nd in (32, 128):
+            for C in (0, 512, 2048):
+                pts.append((f"CTX:{C},1,{nd},m{med}", lambda C=C, nd=nd, med=med: wl.config_c3(C, 1, nd, ctx_median=med)))
+    for name in sorted(wl.SCENE_EDGES):                    # pure-prefill scene edges (tensor-bound)
+        pts.append((name, lambda name=name: wl.config_scene_edge(name)))
+    for name in ("PD-32", "PD-128", "PD-C2", "PD-C5"):     # pure-decode scene edges
+        pts.append((name, lambda name=name: wl.config_decode_only(name)))
+    pts.append(("C2", wl.config_c2))
+    pts.append(("C2-shuffled", lambda: wl.config_c2(shuffle=True)))
+    pts.append(("C5", wl.config_c5))
+    if with_c4:
+        pts.append(("C4", wl.config_c4))
+    return pts
+
+
+def sub_batch(b: wl.Batch, kind: str) -> Optional[wl.Batch]:
+    """The prefill-only (c > 1) or decode-only (c == 1) part of a mixed batch, re-paged on its own pool."""
+    reqs = [(c, u) for c, u in b.reqs if (c > 1 if kind == "prefill" else c == 1)]
+    if not reqs:
+        return None
+    return wl.make_batch(f"{b.name}/{kind}", b.num_q_heads, b.num_kv_heads, b.head_dim, reqs, b.seed + 1,
+                         with_append=False)
+
+
+def time_batch(b: wl.Batch, device: str, iters: int, warmup: int, flush) -> np.ndarray:
+    """us per ss_mixed_attention call (work list + main launch), one sample per timed iteration."""
+    import torch
+    from . import binding
+    t = wl.make_tensors(b, device)
+    h = binding.handle_for(b, t)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    out = torch.empty_like(t.q)
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        flush.fill_(1)
+        binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale, out=out)
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
+    for e0, e1 in evs:
+        flush.fill_(1)
+        e0.record(stream)
+        binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale, out=out)
+        e1.record(stream)
+    torch.cuda.synchronize()
+    us = np.array([e0.elapsed_time(e1) * 1e3 for e0, e1 in evs])
+    h.close()
+    del t, out, h
+    torch.cuda.empty_cache()
+    return us
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--out", default="gpurun_out/surface.csv")
+    ap.add_argument("--iters", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--with-c4", action="store_true", help="include the 40 GB-pool decode-heavy config")
+    ap.add_argument("--only", default=None, help="comma-separated point-id prefixes")
+    args = ap.parse_args(argv)
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("surface sweep needs a CUDA device: the product path has no CPU fallback")
+    device = "cuda:0"
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)
+    peaks = acc.load_peaks()
+    Path(args.out).parent.mkdir(parents=True, exist_ok=True)
+    with open(args.out, "w", newline="") as f:
+        wr = csv.DictWriter(f, fieldnames=FIELDS)
+        wr.writeheader()
+        for pid, make in surface_points(args.with_c4):
+            if args.only and not any(pid.startswith(p) for p in args.only.split(",")):
+                continue
+            b = make()
+            us = time_batch(b, device, args.iters, args.warmup, flush)
+            w, roof, x = acc.work(b), acc.roofline_us(b, peaks), features(b.reqs)
+            row = {"point": pid, "name": b.name, "seed": b.seed, "shape": f"{b.num_q_heads}/{b.num_kv_heads}/{b.head_dim}",
+                   "scene": scene(b.reqs), "R": b.R, "T": b.T, "chunk": b.meta.get("chunk", x["x6"]),
+                   "n_prefill": sum(1 for c, _ in b.reqs if c > 1), "n_decode": x["x4"],
+                   "ctx_median": b.meta.get("ctx_median", ""), **x, "bytes": w["bytes"], "flops": w["flops"],
+                   "t_hbm_us": round(roof["t_hbm_us"], 2), "t_tc_us": round(roof["t_tc_us"], 2),
+                   "roofline_us": round(roof["roofline_us"], 2), "bound": roof["bound"],
+                   "median_us": round(float(np.median(us)), 2), "p10_us": round(float(np.percentile(us, 10)), 2),
+                   "p90_us": round(float(np.percentile(us, 90)), 2),
+                   "frac_of_roofline": round(roof["roofline_us"] / float(np.median(us)), 4),
+                   "prefill_only_us": "", "decode_only_us": "", "overlap": ""}
+            if scene(b.reqs) == "mixed":
+                tp = float(np.median(time_batch(sub_batch(b, "prefill"), device, args.iters, args.warmup, flush)))
+                td = float(np.median(time_batch(sub_batch(b, "decode"), device, args.iters, args.warmup, flush)))
+                row.update(prefill_only_us=round(tp, 2), decode_only_us=round(td, 2),
+                           overlap=round(float(np.median(us)) / (tp + td), 4))
+            wr.writerow(row)
+            f.flush()
+            print(pid, row["median_us"], row["roofline_us"], row["frac_of_roofline"], row["overlap"], file=sys.stderr, flush=True)
+
+
+if __name__ == "__main__":
+    main()
