@@ -160,9 +160,11 @@ int ss_debug_force_simple_path(ss_handle* h, int on);
 int ss_debug_set_param(ss_handle* h, int which, int value);
 
 /* Measurement aid: per-CTA timeline of the main launch.  `trace_dev` is a DEVICE buffer of
- * num_ctas * words_per_cta uint64 words (caller-owned; NULL switches tracing off).  Per CTA the kernel writes
- * word 0 = %globaltimer at entry (ns), 1 = after setup + grid dependency wait, 2 = at exit, 3 = item count, then
- * 3 words per item (start ns, end ns, kind << 32 | KV tiles) while they fit.  Results never depend on it. */
+ * num_ctas * words_per_cta uint64 words (caller-owned; NULL switches tracing off; words_per_cta >= 6).  Per CTA the
+ * kernel writes word 0 = %globaltimer at entry (ns), 1 = after setup + grid dependency wait, 2 = worker warps' exit,
+ * 3 = item count, 4 = exit of the MMA / split-merge warp, 5 = unused, then 9 words per item while they fit: start ns,
+ * end ns, kind << 32 | KV tiles, first tile ready ns, tile loop end ns, and 4 epilogue stamps (decode items only).
+ * Results never depend on it. */
 int ss_debug_set_trace(ss_handle* h, void* trace_dev, int32_t words_per_cta);
 
 const char* ss_status_string(int status);

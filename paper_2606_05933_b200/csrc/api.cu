@@ -194,7 +194,7 @@ int ss_debug_set_param(ss_handle* hh, int which, int value) {
 
 int ss_debug_set_trace(ss_handle* hh, void* trace_dev, int32_t words_per_cta) {
     Handle* h = (Handle*)hh;
-    if (!h || (trace_dev && words_per_cta < 4) || (((uintptr_t)trace_dev) & 7u)) return SS_ERR_INVALID_ARG;
+    if (!h || (trace_dev && words_per_cta < 6) || (((uintptr_t)trace_dev) & 7u)) return SS_ERR_INVALID_ARG;
     h->trace = (unsigned long long*)trace_dev;
     h->trace_words = trace_dev ? words_per_cta : 0;
     return SS_OK;

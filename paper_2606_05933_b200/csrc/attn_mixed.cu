@@ -43,9 +43,15 @@ struct MixSmem {
     static constexpr int kTile = kHalves * kTileKeys * 128;      // one K (or V, or Q) tile
     static constexpr int kKOff = 0;
     static constexpr int kVOff = kKOff + kNumSt * kTile;
-    static constexpr int kQOff = kVOff + kNumSt * kTile;         // Q tile (prefill) / cross-warp merge buffer (decode)
+    static constexpr int kQOff = kVOff + kNumSt * kTile;         // Q tile (prefill) / decode: cross-warp merge buffer + staged Q rows
     static constexpr int kMergeBytes = 4 * kMaxGroup * (D + 2) * 4;
+    // decode with G <= 8: merge buffer of 8 rows per warp, then kSchedSlots staged Q blocks (G rows x D bf16, one per
+    // scheduler slot, bulk-copied by the producer so the workers never wait on a cold global Q load)
+    static constexpr int kMerge8Bytes = 4 * 8 * (D + 2) * 4;
+    static constexpr int kQStageOff = kQOff + (kMerge8Bytes + 127) / 128 * 128;
+    static constexpr int kQStageBytes = 8 * D * 2;
     static constexpr int kQBytes = ((kTile > kMergeBytes ? kTile : kMergeBytes) + 1023) / 1024 * 1024;
+    static_assert(kQStageOff + kSchedSlots * kQStageBytes <= kQOff + kQBytes, "staged Q blocks must fit beside the merge buffer");
     static constexpr int kBarOff = kQOff + kQBytes;
     static constexpr int kSchedOff = kBarOff + 320;              // kSchedSlots x 48 B
     static constexpr int kTmemSlotOff = kSchedOff + kSchedSlots * 48;
@@ -60,7 +66,7 @@ struct MixSmem {
 enum : int {
     B_KFULL = 0, B_VFULL = 3, B_KEMPTY_P = 6, B_KEMPTY_D = 9, B_VEMPTY_P = 12, B_VEMPTY_D = 15,
     B_SFULL = 18, B_PFULL = 20, B_QFULL = 22, B_QEMPTY = 23, B_OFULL = 24, B_OFREE = 25, B_PVDONE = 26,
-    B_SCHED_FULL = 27, B_SCHED_EMPTY = 31, B_COUNT = 35
+    B_SCHED_FULL = 27, B_SCHED_EMPTY = 31, B_PARTIAL = 35, B_COUNT = 39
 };
 static_assert(B_COUNT * 8 <= 320, "barrier region");
 
@@ -132,6 +138,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         mbar_init(BAR(B_OFREE), 128);
         mbar_init(BAR(B_PVDONE), 1);
         for (int s = 0; s < kSchedSlots; ++s) {
+            mbar_init(BAR(B_PARTIAL + s), 128);
             mbar_init(BAR(B_SCHED_FULL + s), 1);
             mbar_init(BAR(B_SCHED_EMPTY + s), 5);
         }
@@ -164,12 +171,10 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             uint32_t parP = 0, parD = 0, lastT = 0;
             uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0;
             int prev_kind = 0;
-            for (;;) {
-                const int slot = n_sched % kSchedSlots;
-                mbar_wait(BAR(B_SCHED_EMPTY + slot), ((n_sched / kSchedSlots) & 1) ^ 1);
-                uint4* dst = reinterpret_cast<uint4*>(smem + SM::kSchedOff + slot * 48);
-                union { ss_work_item it; uint4 v[3]; } wu;
-                // two typed queues: this CTA drains its preferred kind first, then helps with the other
+            const bool q_staged = G <= 8;
+            union WU { ss_work_item it; uint4 v[3]; };
+            // two typed queues: this CTA drains its preferred kind first, then helps with the other
+            auto fetch = [&](WU& wu) {
                 int idx = -1;
                 if (prefer_decode) {
                     if (!dec_done) { const int i = atomicAdd(&prm.hdr->next_decode, 1); if (i < n_dec) idx = n_pre_items + i; else dec_done = true; }
@@ -184,19 +189,47 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 } else {
                     wu.v[0] = wu.v[1] = wu.v[2] = make_uint4(0u, 0u, 0u, 0u);
                 }
+            };
+            auto first_pages = [&](const ss_work_item& it, int (&pgs)[8]) {
+                const int32_t* b = prm.block_table + (int64_t)it.req * prm.max_pages;
+#pragma unroll
+                for (int p = 0; p < 8; ++p)
+                    pgs[p] = (it.kind != 0 && it.kv_begin + p * kPage < it.kv_end) ? __ldg(b + (it.kv_begin >> 4) + p) : 0;
+            };
+            // the NEXT item (queue ticket, record, first page ids) is fetched while the current item's tiles are being
+            // issued, so the atomic -> record -> block-table latency chain never sits between two items' TMA streams
+            WU nxt;
+            int nxt_pg[8];
+            fetch(nxt);
+            first_pages(nxt.it, nxt_pg);
+            for (;;) {
+                const int slot = n_sched % kSchedSlots;
+                mbar_wait(BAR(B_SCHED_EMPTY + slot), ((n_sched / kSchedSlots) & 1) ^ 1);
+                uint4* dst = reinterpret_cast<uint4*>(smem + SM::kSchedOff + slot * 48);
+                const WU wu = nxt;
                 dst[0] = wu.v[0]; dst[1] = wu.v[1]; dst[2] = wu.v[2];
-                mbar_arrive(BAR(B_SCHED_FULL + slot));        // release semantics: the item is visible to the waiters
                 const ss_work_item& w = wu.it;
+                if (w.kind == 2 && q_staged) {
+                    // the staged Q block lies inside the prefill Q tile: the last prefill item's S MMAs must be done
+                    mbar_wait(BAR(B_QEMPTY), (n_pre & 1) ^ 1);
+                    const uint32_t qbytes = (uint32_t)(G * D * 2);
+                    mbar_arrive_expect_tx(BAR(B_SCHED_FULL + slot), qbytes);     // release: the record is visible too
+                    bulk_load_1d(sbase + SM::kQStageOff + slot * SM::kQStageBytes,
+                                 prm.q + ((int64_t)w.row0 * Hq + (int64_t)w.head * G) * D, qbytes, BAR(B_SCHED_FULL + slot));
+                } else {
+                    mbar_arrive(BAR(B_SCHED_FULL + slot));        // release semantics: the item is visible to the waiters
+                }
                 ++n_sched;
                 if (w.kind == 0) break;
                 const int32_t* bt = prm.block_table + (int64_t)w.req * prm.max_pages;
                 const int g = w.kind == 1 ? w.head / G : w.head;
                 int pg[8];
+#pragma unroll
+                for (int p = 0; p < 8; ++p) pg[p] = nxt_pg[p];
                 auto load_pages = [&](int key0) {
 #pragma unroll
                     for (int p = 0; p < 8; ++p) pg[p] = (key0 + p * kPage < w.kv_end) ? __ldg(bt + (key0 >> 4) + p) : 0;
                 };
-                load_pages(w.kv_begin);
                 if (w.kind == 1) {
                     mbar_wait(BAR(B_QEMPTY), (n_pre & 1) ^ 1);
                     if (prev_kind == 2) {
@@ -212,6 +245,12 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 }
                 prev_kind = w.kind;
                 for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kTileKeys, ++tile_ctr) {
+                    if (key0 + kTileKeys >= w.kv_end) {
+                        // last tile of this item: draw the next ticket now (not earlier, or the tail of the launch
+                        // grows by an item held while this one is still streaming); the ring hides the chain
+                        fetch(nxt);
+                        first_pages(nxt.it, nxt_pg);
+                    }
                     const int s = tile_ctr % kNumSt;
                     const int npages = min(8, (w.kv_end - key0 + kPage - 1) / kPage);
                     const uint32_t bytes = (uint32_t)npages * kHalves * 2048;
@@ -250,33 +289,37 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         }
     } else if (warp == 1) {
         // =============================== tcgen05.mma issuer ===============================
-        // One elected thread runs the whole loop (waits included): descriptors stay in uniform registers.
-        if (elect_one()) {
-            constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kTileKeys, 0);
-            constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileRows, D, 1);
-            const uint64_t qdesc0 = umma_desc_sw128(sbase + SM::kQOff, 16, 1024);
-            uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_pre = 0;
-            auto issue_s = [&](uint32_t tc, uint32_t sc) {
-                const int s = tc % kNumSt, b = sc & 1;
-                mbar_wait(BAR(B_KFULL + s), (tc / kNumSt) & 1);
-                tc_fence_after();
-                const uint64_t kdesc0 = umma_desc_sw128(sbase + SM::kKOff + s * SM::kTile, 16, 1024);
+        // Prefill items: one elected thread issues every MMA of the item (waits included), so descriptors stay in
+        // uniform registers.  Decode items: this warp is idle on the data path, so it runs a5 for the workers: it
+        // publishes each split partial (acq_rel ticket) and merges the splits of a (request, kv head) when it draws
+        // the last ticket - off the workers' critical path.
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kTileKeys, 0);
+        constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileRows, D, 1);
+        uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_pre = 0;
+        for (;;) {
+            const int slot = n_sched % kSchedSlots;
+            mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
+            const ss_work_item w = sched[slot];
+            const int kind = w.kind;
+            const int ntiles = (w.kv_end - w.kv_begin + kTileKeys - 1) / kTileKeys;
+            ++n_sched;
+            if (kind == 0) break;
+            if (kind == 1) {
+                if (elect_one()) {
+                    const uint64_t qdesc0 = umma_desc_sw128(sbase + SM::kQOff, 16, 1024);
+                    auto issue_s = [&](uint32_t tc, uint32_t sc) {
+                        const int s = tc % kNumSt, b = sc & 1;
+                        mbar_wait(BAR(B_KFULL + s), (tc / kNumSt) & 1);
+                        tc_fence_after();
+                        const uint64_t kdesc0 = umma_desc_sw128(sbase + SM::kKOff + s * SM::kTile, 16, 1024);
 #pragma unroll
-                for (int ks = 0; ks < D / 16; ++ks) {
-                    const uint32_t off = (ks >> 2) * (kTileRows * 128) + (ks & 3) * 32;      // bytes; descriptor address unit = 16 B
-                    umma_ss(tmem_base + b * 128, qdesc0 + (off >> 4), kdesc0 + (off >> 4), idesc_qk, ks > 0);
-                }
-                umma_commit(BAR(B_KEMPTY_P + s));
-                umma_commit(BAR(B_SFULL + b));
-            };
-            for (;;) {
-                const int slot = n_sched % kSchedSlots;
-                mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
-                const int kind = sched[slot].kind;
-                const int ntiles = (sched[slot].kv_end - sched[slot].kv_begin + kTileKeys - 1) / kTileKeys;
-                ++n_sched;
-                if (kind == 0) break;
-                if (kind == 1) {
+                        for (int ks = 0; ks < D / 16; ++ks) {
+                            const uint32_t off = (ks >> 2) * (kTileRows * 128) + (ks & 3) * 32;      // bytes; descriptor address unit = 16 B
+                            umma_ss(tmem_base + b * 128, qdesc0 + (off >> 4), kdesc0 + (off >> 4), idesc_qk, ks > 0);
+                        }
+                        umma_commit(BAR(B_KEMPTY_P + s));
+                        umma_commit(BAR(B_SFULL + b));
+                    };
                     mbar_wait(BAR(B_QFULL), n_pre & 1);
                     issue_s(tile_ctr, s_ctr);
                     for (int t = 0; t < ntiles; ++t) {
@@ -296,13 +339,71 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         umma_commit(BAR(B_PVDONE));
                         if (t == ntiles - 1) umma_commit(BAR(B_OFULL));
                     }
-                    s_ctr += ntiles;
-                    ++n_pre;
                 }
-                tile_ctr += ntiles;
-                mbar_arrive(BAR(B_SCHED_EMPTY + slot));
+                __syncwarp();
+                s_ctr += ntiles;
+                ++n_pre;
+            } else if (w.nsplit > 1) {
+                // ---- a5: publish this split; the last ticket of (request, kv head) merges in fixed split order ----
+                mbar_wait(BAR(B_PARTIAL + slot), ((n_sched - 1) / kSchedSlots) & 1);   // acquire (CTA): all 128 workers' partial stores
+                int last = 0;
+                if (lane == 0) last = atom_add_acq_rel_gpu(prm.merge_counters + w.req * Hkv + w.head, 1) == w.nsplit - 1;
+                last = __shfl_sync(0xffffffffu, last, 0);
+                __syncwarp();
+                if (last) {
+                    // lane owns columns d = lane + 32 j; 4 rows (q heads) per pass; per split 8 + 4 D/32 independent
+                    // L2 loads in flight per lane, online log-sum-exp merge in split order
+                    constexpr int DJ = D / 32;
+                    const int64_t sstride = (int64_t)G * (D + 2);
+                    const float* pbase = prm.partials + (int64_t)w.partial * sstride;
+                    for (int r0 = 0; r0 < G; r0 += 4) {
+                        float M[4], L[4], A[4][DJ];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            M[i] = -INFINITY; L[i] = 0.f;
+#pragma unroll
+                            for (int j = 0; j < DJ; ++j) A[i][j] = 0.f;
+                        }
+#pragma unroll 2
+                        for (int x = 0; x < w.nsplit; ++x) {
+                            const float* px = pbase + x * sstride;
+                            float mx[4], lx[4], ox[4][DJ];
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                const float* pr = px + min(r0 + i, G - 1) * (D + 2);
+                                mx[i] = __ldcg(pr + D);
+                                lx[i] = __ldcg(pr + D + 1);
+#pragma unroll
+                                for (int j = 0; j < DJ; ++j) ox[i][j] = __ldcg(pr + lane + 32 * j);
+                            }
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                const float Mn = fmaxf(M[i], mx[i]);
+                                const float al = exp2f(M[i] - Mn), bx = exp2f(mx[i] - Mn);
+                                L[i] = L[i] * al + lx[i] * bx;
+#pragma unroll
+                                for (int j = 0; j < DJ; ++j) A[i][j] = A[i][j] * al + ox[i][j] * bx;
+                                M[i] = Mn;
+                            }
+                        }
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            if (r0 + i < G) {
+                                const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r0 + i;
+                                const float inv = 1.f / L[i];
+#pragma unroll
+                                for (int j = 0; j < DJ; ++j) prm.out[orow * D + lane + 32 * j] = __float2bfloat16_rn(A[i][j] * inv);
+                                if (prm.lse && lane == 0) prm.lse[orow] = (M[i] + log2f(L[i])) * kMLn2;
+                            }
+                        }
+                    }
+                }
             }
+            tile_ctr += ntiles;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
         }
+        if (trace && lane == 0) trace[4] = globaltimer_ns();
     } else {
         // =============================== workers ===============================
         const int cw = warp - 2;                               // decode: key slice; also == TMEM lane quarter order below
@@ -315,6 +416,8 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_pre = 0;
         float* merge = reinterpret_cast<float*>(smem + SM::kQOff);
         int* flag = reinterpret_cast<int*>(smem + SM::kTmemSlotOff + 16);
+        const bool q_staged = G <= 8;
+        const int mrows = q_staged ? 8 : kMaxGroup;           // merge-buffer rows per warp
         for (;;) {
             const int slot = n_sched % kSchedSlots;
             mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
@@ -322,9 +425,10 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             ++n_sched;
             if (w.kind == 0) break;
             const int ntiles = (w.kv_end - w.kv_begin + kTileKeys - 1) / kTileKeys;
-            if (trace && wtid == 0 && 4 + 3 * (int)n_sched <= prm.trace_words) {
-                trace[4 + 3 * (n_sched - 1)] = globaltimer_ns();
-                trace[4 + 3 * (n_sched - 1) + 2] = ((unsigned long long)w.kind << 32) | (unsigned)ntiles;
+            unsigned long long* const tr = (trace && wtid == 0 && 6 + 9 * (int)n_sched <= prm.trace_words) ? trace + 6 + 9 * (n_sched - 1) : nullptr;
+            if (tr) {
+                tr[0] = globaltimer_ns();
+                tr[2] = ((unsigned long long)w.kind << 32) | (unsigned)ntiles;
             }
             if (w.kind == 1) {
                 // -------------------------- prefill tile: thread = query row --------------------------
@@ -349,6 +453,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     }
                     mbar_wait(BAR(B_SFULL + b), (sc >> 1) & 1);
                     tc_fence_after();
+                    if (tr && t == 0) tr[3] = globaltimer_ns();
                     uint32_t sr[4][32];
 #pragma unroll
                     for (int c = 0; c < 4; ++c) tmem_ld_32x32b_x32(tmem_base + b * 128 + lane_addr + c * 32, sr[c]);
@@ -408,6 +513,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     mbar_arrive(BAR(B_PFULL + b));
                 }
                 // ---- epilogue ----
+                if (tr) tr[4] = globaltimer_ns();
                 mbar_wait(BAR(B_OFULL), n_pre & 1);
                 tc_fence_after();
                 const float inv = 1.f / l;
@@ -433,12 +539,22 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 if (store && prm.lse) prm.lse[(int64_t)(w.row0 + row) * Hq + w.head] = (m + log2f(l)) * kMLn2;
                 tc_fence_before();
                 mbar_arrive(BAR(B_OFREE));
+                mbar_arrive(BAR(B_PARTIAL + slot));               // keeps the per-slot phase count in step (decode-only use)
                 s_ctr += ntiles;
                 ++n_pre;
             } else {
                 // -------------------------- decode split: warp = 32-key slice --------------------------
                 uint32_t qa[D / 16][4];
-                {
+                if (q_staged) {
+                    const uint32_t qs = sbase + SM::kQStageOff + slot * SM::kQStageBytes + (qrow * D + qcol) * 2;
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        qa[ks][0] = qrow < G ? lds32(qs + ks * 32) : 0u;
+                        qa[ks][2] = qrow < G ? lds32(qs + ks * 32 + 16) : 0u;
+                        qa[ks][1] = 0u;
+                        qa[ks][3] = 0u;
+                    }
+                } else {
                     const __nv_bfloat16* qb = prm.q + ((int64_t)w.row0 * Hq + (int64_t)w.head * G) * D;
 #pragma unroll
                     for (int ks = 0; ks < D / 16; ++ks) {
@@ -463,6 +579,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     const uint32_t vbase = sbase + SM::kVOff + s * SM::kTile;
                     float sacc[4][4];
                     mbar_wait(BAR(B_KFULL + s), fpar);
+                    if (tr && t == 0) tr[3] = globaltimer_ns();
                     if (nvalid > 0) {
 #pragma unroll
                         for (int nt = 0; nt < 4; ++nt) sacc[nt][0] = sacc[nt][1] = sacc[nt][2] = sacc[nt][3] = 0.f;
@@ -544,32 +661,36 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     if (lane == 0) mbar_arrive(BAR(B_VEMPTY_D + s));
                 }
                 // ---- cross-warp log-sum-exp merge through smem ----
+                if (tr) tr[4] = globaltimer_ns();
                 l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
                 l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
                 l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
                 l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
-                float* mine = merge + cw * kMaxGroup * (D + 2);
+                float* mine = merge + cw * mrows * (D + 2);
 #pragma unroll
                 for (int i = 0; i < D / 8; ++i) {
                     *reinterpret_cast<float2*>(mine + qrow * (D + 2) + i * 8 + qcol) = make_float2(o[i][0], o[i][1]);
-                    *reinterpret_cast<float2*>(mine + (qrow + 8) * (D + 2) + i * 8 + qcol) = make_float2(o[i][2], o[i][3]);
+                    if (!q_staged) *reinterpret_cast<float2*>(mine + (qrow + 8) * (D + 2) + i * 8 + qcol) = make_float2(o[i][2], o[i][3]);
                 }
                 if ((lane & 3) == 0) {
                     mine[qrow * (D + 2) + D] = m0;
                     mine[qrow * (D + 2) + D + 1] = l0;
-                    mine[(qrow + 8) * (D + 2) + D] = m1;
-                    mine[(qrow + 8) * (D + 2) + D + 1] = l1;
+                    if (!q_staged) {
+                        mine[(qrow + 8) * (D + 2) + D] = m1;
+                        mine[(qrow + 8) * (D + 2) + D + 1] = l1;
+                    }
                 }
                 named_bar_sync(1, 128);
+                if (tr) tr[5] = globaltimer_ns();
                 for (int e = wtid; e < G * D; e += 128) {
                     const int r = e / D, d = e % D;
                     float M = -INFINITY;
 #pragma unroll
-                    for (int x = 0; x < 4; ++x) M = fmaxf(M, merge[(x * kMaxGroup + r) * (D + 2) + D]);
+                    for (int x = 0; x < 4; ++x) M = fmaxf(M, merge[(x * mrows + r) * (D + 2) + D]);
                     float L = 0.f, acc = 0.f;
 #pragma unroll
                     for (int x = 0; x < 4; ++x) {
-                        const float* src = merge + (x * kMaxGroup + r) * (D + 2);
+                        const float* src = merge + (x * mrows + r) * (D + 2);
                         const float wgt = exp2f(src[D] - M);
                         L += src[D + 1] * wgt;
                         acc += src[d] * wgt;
@@ -584,39 +705,15 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         if (d == 0) { dst[D] = M; dst[D + 1] = L; }
                     }
                 }
-                if (w.nsplit > 1) {
-                    // ---- a5: the CTA that completes the last split of (req, kv head) merges all splits ----
-                    __threadfence();
-                    named_bar_sync(1, 128);
-                    if (wtid == 0) {
-                        const int old = atomicAdd(prm.merge_counters + w.req * Hkv + w.head, 1);
-                        *flag = (old == w.nsplit - 1);
-                    }
-                    named_bar_sync(1, 128);
-                    if (*flag) {
-                        __threadfence();
-                        for (int e = wtid; e < G * D; e += 128) {
-                            const int r = e / D, d = e % D;
-                            const float* base = prm.partials + ((int64_t)w.partial * G + r) * (D + 2);
-                            const int64_t sstride = (int64_t)G * (D + 2);
-                            float M = -INFINITY;
-                            for (int x = 0; x < w.nsplit; ++x) M = fmaxf(M, __ldcg(base + x * sstride + D));
-                            float L = 0.f, acc = 0.f;
-                            for (int x = 0; x < w.nsplit; ++x) {
-                                const float wgt = exp2f(__ldcg(base + x * sstride + D) - M);
-                                L += __ldcg(base + x * sstride + D + 1) * wgt;
-                                acc += __ldcg(base + x * sstride + d) * wgt;
-                            }
-                            const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r;
-                            prm.out[orow * D + d] = __float2bfloat16_rn(acc / L);
-                            if (prm.lse && d == 0) prm.lse[orow] = (M + log2f(L)) * kMLn2;
-                        }
-                    }
-                }
-                named_bar_sync(1, 128);
+                if (tr) tr[6] = globaltimer_ns();
+                // a5 hand-off: the (otherwise idle) MMA warp publishes this split and, if it was the last of its
+                // (request, kv head), merges all of them; the workers go straight on to the next item.  mbarrier
+                // arrive = release at CTA scope for this thread's partial stores.
+                mbar_arrive(BAR(B_PARTIAL + slot));           // once per item and slot use (phase = slot use count)
+                named_bar_sync(1, 128);                       // merge buffer free for the next item
             }
             tile_ctr += ntiles;
-            if (trace && wtid == 0 && 4 + 3 * (int)n_sched <= prm.trace_words) trace[4 + 3 * (n_sched - 1) + 1] = globaltimer_ns();
+            if (tr) tr[1] = globaltimer_ns();
             __syncwarp();
             if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
         }
