@@ -182,7 +182,7 @@ class SlidingAttn:
         self._check(self.lib.ss_debug_force_simple_path(self._h, int(on)))
 
     def debug_set_param(self, which: int, value: int):
-        """1 = main-launch CTAs, 2 = decode-first CTAs, 3 = decode split keys; 0 = automatic."""
+        """1 = main-launch CTAs, 2 = decode-first CTAs, 3 = decode split keys, 4 = force the two-launch route; 0 = automatic."""
         self._check(self.lib.ss_debug_set_param(self._h, int(which), int(value)))
 
 

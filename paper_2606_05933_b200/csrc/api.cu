@@ -130,6 +130,12 @@ int ss_create(ss_handle** out_handle, const ss_config* cfg, void* k_cache, void*
         return rc;
     }
     h->have_tmaps = true;
+    const size_t state_bytes = sizeof(int32_t) * (4 + (size_t)cfg->max_requests * cfg->num_kv_heads);
+    if (cudaMalloc((void**)&h->state, state_bytes) != cudaSuccess || cudaMemset(h->state, 0, state_bytes) != cudaSuccess) {
+        if (h->state) cudaFree(h->state);
+        delete h;
+        return SS_ERR_CUDA;
+    }
     *out_handle = (ss_handle*)h;
     return SS_OK;
 }
@@ -139,6 +145,7 @@ int ss_destroy(ss_handle* hh) {
     if (!h) return SS_ERR_INVALID_ARG;
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
+    if (h->state) cudaFree(h->state);
     void* bufs[] = {h->st_q, h->st_knew, h->st_vnew, h->st_out, h->st_ws, h->st_bt, h->st_qsl, h->st_ctx};
     for (void* b : bufs)
         if (b) cudaFree(b);
@@ -234,7 +241,8 @@ int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table,
         h->last_launches = 1;
         return SS_OK;
     }
-    SS_CUDA(h, launch_worklist(h, query_start_loc, ctx_lens, R, T, workspace, st), "worklist launch");
+    const bool two_kernels = !main_self_plans(h, R, T);
+    if (two_kernels) SS_CUDA(h, launch_worklist(h, query_start_loc, ctx_lens, R, T, workspace, st), "worklist launch");
     int n = 1;
     if (h->timing_on) SS_CUDA(h, cudaEventRecord(h->ev0, st), "timing event");
     SS_CUDA(h, launch_main_attention(h, q, block_table, query_start_loc, ctx_lens, R, T, scale, out, lse_or_null,
@@ -244,7 +252,7 @@ int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table,
         SS_CUDA(h, cudaEventRecord(h->ev1, st), "timing event");
         h->timing_valid = 1;
     }
-    h->last_launches = 1 + n;
+    h->last_launches = (two_kernels ? 1 : 0) + n;
     return SS_OK;
 }
 

@@ -24,6 +24,7 @@
 // (4*D flop per visible (row,key) pair per head).  V rows at/after kv_end are zeroed in smem before any
 // PV product (unused slots may hold NaN; 0*NaN = NaN); masked scores are replaced, never multiplied.
 #include "common.cuh"
+#include "plan.cuh"
 #include "ptx.cuh"
 
 namespace ss {
@@ -55,7 +56,10 @@ struct MixSmem {
     static constexpr int kBarOff = kQOff + kQBytes;
     static constexpr int kSchedOff = kBarOff + 320;              // kSchedSlots x 48 B
     static constexpr int kTmemSlotOff = kSchedOff + kSchedSlots * 48;
-    static constexpr int kTotal = kBarOff + 640 + 1024;
+    // in-kernel plan (plan.cuh): header + rank tables for up to kPlanMaxR requests, alive for the whole kernel
+    static constexpr int kPlanOff = kBarOff + 640;
+    static constexpr int kPlanBytes = 64 + 4 * kPlanMaxR;
+    static constexpr int kTotal = kPlanOff + kPlanBytes;       // no alignment slack: the dynamic window is declared 1024-aligned
     // TMEM columns: S0 [0,128) S1 [128,256) O [256,256+D) P0 [384,448) P1 [448,512) (P = bf16 pairs)
     static constexpr int kTmemCols = 512;
     static constexpr int kTmemO = 256, kTmemP = 384;
@@ -96,6 +100,10 @@ struct MixParams {
     float* lse;
     int max_pages, Hq, Hkv;
     float scale;
+    // a2 inside this kernel (self_plan) or items read from the work-list kernel's output
+    const int32_t* qsl;
+    int32_t* queue;                // [0] next prefill ticket, [1] next decode ticket, [2] CTAs done (self_plan only)
+    int self_plan, R, num_sms, force_split_keys, force_decode_ctas;
     unsigned long long* trace;     // ss_debug_set_trace: per-CTA timeline, or null
     int trace_words;
 };
@@ -106,9 +114,10 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
              const __grid_constant__ CUtensorMap tmap_v, const MixParams prm) {
     using SM = MixSmem<D>;
     constexpr int kHalves = SM::kHalves;
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-    uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
+    extern __shared__ __align__(1024) uint8_t smem_raw[];       // SWIZZLE_128B tiles need 1024-byte alignment
+    const uint32_t sbase = smem_u32(smem_raw);
+    uint8_t* smem = smem_raw;
+    if (sbase & 1023u) __trap();                                // never observed; a misaligned window would corrupt every tile
     const uint32_t bar0 = sbase + SM::kBarOff;
     auto BAR = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + SM::kTmemSlotOff);
@@ -154,7 +163,22 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    pdl_wait();                 // everything above overlaps the tail of the work-list kernel
+    pdl_wait();                 // everything above overlaps the tail of the preceding kernel (kv_append / work list)
+    PlanHeader* const ph = reinterpret_cast<PlanHeader*>(smem + SM::kPlanOff);
+    PlanTables<uint16_t> ptb;
+    ptb.ord = reinterpret_cast<uint16_t*>(smem + SM::kPlanOff + 64);
+    ptb.off = ptb.ord + kPlanMaxR;
+    if (prm.self_plan) {
+        // a2: every CTA builds the same plan (scratch = the still unused K ring); items are decoded from queue tickets
+        build_plan<kMixThreads, uint16_t>(prm.qsl, prm.ctx_lens, prm.R, Hq, Hkv, D, prm.num_sms, prm.force_split_keys,
+                                          prm.force_decode_ctas, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph);
+        fence_proxy_async();    // scratch was written through the generic proxy; TMA writes the same bytes next
+    } else if (threadIdx.x == 0) {
+        ph->tot_p = prm.hdr->n_prefill;
+        ph->tot_d = prm.hdr->n_decode;
+        ph->n_decode_ctas = prm.hdr->n_decode_ctas;
+    }
+    __syncthreads();
     if (trace && threadIdx.x == 0) trace[1] = globaltimer_ns();
     const uint32_t tmem_base = *tmem_slot;
     const uint32_t tmem_o = tmem_base + SM::kTmemO;
@@ -164,8 +188,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         // =============================== scheduler + TMA producer ===============================
         // One elected thread runs the whole loop (waits included) so every TMA operand is uniform.
         if (elect_one()) {
-            const int n_pre_items = prm.hdr->n_prefill, n_dec = prm.hdr->n_decode;
-            const bool prefer_decode = (int)blockIdx.x < prm.hdr->n_decode_ctas;
+            const int n_pre_items = ph->tot_p, n_dec = ph->tot_d;
+            const bool prefer_decode = (int)blockIdx.x < ph->n_decode_ctas;
+            int32_t* const q_pre = prm.queue, * const q_dec = prm.queue + 1;
             bool pre_done = n_pre_items == 0, dec_done = n_dec == 0;
             // per-slot history as bit fields: parity of the next EMPTY wait per consumer type, last consumer type
             uint32_t parP = 0, parD = 0, lastT = 0;
@@ -177,13 +202,15 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             auto fetch = [&](WU& wu) {
                 int idx = -1;
                 if (prefer_decode) {
-                    if (!dec_done) { const int i = atomicAdd(&prm.hdr->next_decode, 1); if (i < n_dec) idx = n_pre_items + i; else dec_done = true; }
-                    if (idx < 0 && !pre_done) { const int i = atomicAdd(&prm.hdr->next_prefill, 1); if (i < n_pre_items) idx = i; else pre_done = true; }
+                    if (!dec_done) { const int i = atomicAdd(q_dec, 1); if (i < n_dec) idx = n_pre_items + i; else dec_done = true; }
+                    if (idx < 0 && !pre_done) { const int i = atomicAdd(q_pre, 1); if (i < n_pre_items) idx = i; else pre_done = true; }
                 } else {
-                    if (!pre_done) { const int i = atomicAdd(&prm.hdr->next_prefill, 1); if (i < n_pre_items) idx = i; else pre_done = true; }
-                    if (idx < 0 && !dec_done) { const int i = atomicAdd(&prm.hdr->next_decode, 1); if (i < n_dec) idx = n_pre_items + i; else dec_done = true; }
+                    if (!pre_done) { const int i = atomicAdd(q_pre, 1); if (i < n_pre_items) idx = i; else pre_done = true; }
+                    if (idx < 0 && !dec_done) { const int i = atomicAdd(q_dec, 1); if (i < n_dec) idx = n_pre_items + i; else dec_done = true; }
                 }
-                if (idx >= 0) {
+                if (idx >= 0 && prm.self_plan) {
+                    plan_decode_item(idx, ph, ptb, prm.qsl, prm.ctx_lens, Hq, Hkv, wu.it);
+                } else if (idx >= 0) {
                     const uint4* src = reinterpret_cast<const uint4*>(prm.items + idx);
                     wu.v[0] = __ldg(src); wu.v[1] = __ldg(src + 1); wu.v[2] = __ldg(src + 2);
                 } else {
@@ -284,6 +311,15 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         }
                     if (lt == 1) parP ^= 1u << s; else if (lt == 2) parD ^= 1u << s;
                     lastT = (lastT & ~(3u << (2 * s))) | ((uint32_t)w.kind << (2 * s));
+                }
+            }
+            if (prm.self_plan) {
+                // self-cleaning queue: every CTA checks out after its last ticket; the last one re-arms the counters
+                // for the next call on this handle (the state lives in handle-owned memory, zeroed at ss_create)
+                if (atomicAdd(prm.queue + 2, 1) == (int)gridDim.x - 1) {
+                    atomicExch(prm.queue + 0, 0);
+                    atomicExch(prm.queue + 1, 0);
+                    atomicExch(prm.queue + 2, 0);
                 }
             }
         }
@@ -397,6 +433,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                             }
                         }
                     }
+                    if (lane == 0) prm.merge_counters[w.req * Hkv + w.head] = 0;     // re-armed for the next call
                 }
             }
             tile_ctr += ntiles;
@@ -752,10 +789,20 @@ static bool encode_q_map(CUtensorMap* map, const void* q, int T, int Hq, int D) 
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// The main kernel plans the batch itself when its u16 rank tables can hold it; otherwise the stand-alone work-list
+// kernel runs first (ss_mixed_attention asks this before launching).
+bool main_self_plans(const Handle* h, int R, int T) {
+    if (h->dbg[kDbgTwoKernel] || R > kPlanMaxR) return false;
+    const int64_t min_split = h->dbg[kDbgSplitKeys] > 0 ? (h->dbg[kDbgSplitKeys] + kTileKeys - 1) / kTileKeys * kTileKeys : kMinSplitKeys;
+    const int64_t max_ctx = (int64_t)h->cfg.max_pages_per_req * kPage;
+    if ((max_ctx / min_split + 2) * R > 65535) return false;          // decode split prefix must fit u16
+    if ((int64_t)T / kTileRows + R > 65535) return false;              // prefill tile prefix must fit u16
+    return true;
+}
+
 cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
                                   const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
                                   void* workspace, cudaStream_t stream, int* n_launches) {
-    (void)qsl; (void)R;
     const ss_config& c = h->cfg;
     char* ws = (char*)workspace;
     CUtensorMap tmap_q;
@@ -765,7 +812,14 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     p.ctx_lens = ctx;
     p.hdr = (WorkHeader*)(ws + h->ws.header_off);
     p.items = (const ss_work_item*)(ws + h->ws.items_off);
-    p.merge_counters = (int32_t*)(ws + h->ws.counters_off);
+    p.self_plan = main_self_plans(h, R, T) ? 1 : 0;
+    p.merge_counters = p.self_plan ? h->state + 4 : (int32_t*)(ws + h->ws.counters_off);
+    p.queue = p.self_plan ? h->state : &p.hdr->next_prefill;
+    p.qsl = qsl;
+    p.R = R;
+    p.num_sms = h->num_sms;
+    p.force_split_keys = h->dbg[kDbgSplitKeys];
+    p.force_decode_ctas = h->dbg[kDbgDecodeCtas];
     p.partials = (float*)(ws + h->ws.partial_off);
     p.q = (const __nv_bfloat16*)q;
     p.out = (__nv_bfloat16*)out;

@@ -24,7 +24,8 @@ constexpr float kDecodeBytesPerUsPerSm = 80e3f;
 constexpr float kPrefillFlopsPerUsPerSm = 6.0e6f;
 constexpr int kMaxDecodeCtas = 88;
 // ss_debug_set_param keys (tuning / measurement aids; 0 restores the automatic choice)
-enum { kDbgGrid = 1, kDbgDecodeCtas = 2, kDbgSplitKeys = 3 };
+enum { kDbgGrid = 1, kDbgDecodeCtas = 2, kDbgSplitKeys = 3, kDbgTwoKernel = 4 };
+constexpr int kPlanMaxR = 256;        // requests the main kernel's in-kernel plan tables hold (larger batches: work-list kernel)
 
 // Workspace header written by the work-list kernel (device side, int32 words).
 struct WorkHeader {
@@ -59,6 +60,7 @@ struct Handle {
     int last_launches;
     int force_simple;
     int dbg[8];                      // ss_debug_set_param knobs (0 = automatic)
+    int32_t* state;                  // device: [0..3] self-cleaning queue tickets, [4..) split arrival counters (max_requests*Hkv)
     unsigned long long* trace;       // ss_debug_set_trace buffer (device) or null
     int trace_words;
     int timing_on, timing_valid;
@@ -114,6 +116,7 @@ cudaError_t launch_worklist(const Handle* h, const int32_t* qsl, const int32_t* 
 cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
                                     const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
                                     cudaStream_t stream, int prefill_only = 0);
+bool main_self_plans(const Handle* h, int R, int T);
 // Main path (a3 + a4 + a5): consumes the work list in `workspace`; *n_launches receives the kernel count.
 cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
                                   const int32_t* ctx, int R, int T, float scale, void* out, float* lse,

@@ -110,6 +110,46 @@ def test_long_context_small_batch_exercises_split_kv():
     full_parity(b)
 
 
+def test_in_kernel_plan_and_two_launch_route_agree_bitwise():
+    """Batches of <= 256 requests are planned inside the main kernel (one launch); larger ones, or debug knob 4, take
+    the stand-alone work-list kernel first.  Same plan functions => bitwise identical outputs; repeated calls on one
+    handle exercise the self-cleaning queue / arrival counters."""
+    b = wl.random_batch(4242, Hq=32, Hkv=8, D=128, n_prefill=3, n_decode=40, max_c=400, max_u=5000)
+    t = wl.make_tensors(b, DEV, poison_unused=True)
+    k0, v0 = wl.to_u16(t.k_cache), wl.to_u16(t.v_cache)
+    out1, lse1, h = gpu_run(b, t)
+    assert h.last_launch_count() == 1
+    out1b, _, _ = gpu_run(wl.Batch(**{**b.__dict__, "with_append": False}), t, handle=h)
+    assert torch.equal(out1, out1b), "second call on the same handle differs (queue state not re-armed?)"
+    h.debug_set_param(4, 1)
+    out2, lse2, _ = gpu_run(wl.Batch(**{**b.__dict__, "with_append": False}), t, handle=h)
+    assert h.last_launch_count() == 2
+    h.debug_set_param(4, 0)
+    assert torch.equal(out1, out2) and torch.equal(lse1, lse2)
+    oracle.kv_append(k0, v0, wl.to_u16(t.k_new), wl.to_u16(t.v_new), b.block_table, b.query_start_loc, b.ctx_lens)
+    ref, lse_ref, _ = oracle.mixed_attention(wl.to_u16(t.q), k0, v0, b.block_table, b.query_start_loc, b.ctx_lens, b.scale)
+    check(b, out2, ref, lse2, lse_ref)
+
+
+def test_more_requests_than_the_in_kernel_plan_holds():
+    rng = np.random.default_rng(5)
+    reqs = [(1, int(u)) for u in rng.integers(0, 300, size=290)] + [(37, 100), (2, 0)]
+    b = wl.make_batch("r292", 8, 2, 128, reqs, 93, with_append=True, shuffle_requests=True)
+    t = wl.make_tensors(b, DEV, poison_unused=True)
+    k0, v0 = wl.to_u16(t.k_cache), wl.to_u16(t.v_cache)
+    out, lse, h = gpu_run(b, t)
+    assert h.last_launch_count() == 2
+    oracle.kv_append(k0, v0, wl.to_u16(t.k_new), wl.to_u16(t.v_new), b.block_table, b.query_start_loc, b.ctx_lens)
+    ref, lse_ref, _ = oracle.mixed_attention(wl.to_u16(t.q), k0, v0, b.block_table, b.query_start_loc, b.ctx_lens, b.scale)
+    check(b, out, ref, lse, lse_ref)
+
+
+def test_group16_shape():
+    reqs = [(140, 50), (1, 2000), (1, 31), (1, 700)]
+    b = wl.make_batch("g16", 32, 2, 128, reqs, 94, with_append=True)
+    full_parity(b)
+
+
 def test_70b_shape_group8():
     reqs = [(130, 77), (1, 3000), (1, 17), (2, 0), (1, 800)]
     b = wl.make_batch("g8", 64, 8, 128, reqs, 92, with_append=True)
@@ -266,7 +306,7 @@ def test_worklist_partitions_the_batch():
                 slots.add(slot)
         covered[b.query_start_loc[r], g * 8:(g + 1) * 8] += 1
     assert len(spans) == sum(1 for c, _ in b.reqs if c == 1) * 8
-    assert len(slots) == n_part
+    assert len(slots) <= n_part          # partial slots share the decode items' index space
     assert (covered == 1).all()
     # heavy-first inside each kind
     assert (np.diff(pre["kv_end"][::64].astype(np.int64)) <= 128).all() or True
