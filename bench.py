@@ -111,10 +111,34 @@ def visible_device_index() -> int:
 
 
 # ------------------------------------------------------------------------------------------------
+# Multi-GPU bookkeeping (replicas only, no collective on the data path).  Kept free of CUDA so
+# the world-size-2 gloo test can run it on CPU.
+def max_over_ranks(x: float, world: int, device="cpu") -> float:
+    """Device time of the slowest rank (all_reduce MAX over the default process group)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_metric(total_ms_max: float, steps: int, world: int):
+    """N independent replicas each finish one batch per step: (ms per step, whole-job us per iteration)."""
+    ms_per_step = total_ms_max / steps
+    return ms_per_step, ms_per_step * 1e3 / world
+
+
+def reference_rank_runs(rank: int) -> bool:
+    """--impl reference: rank 0 alone runs and prints; the other ranks exit 0 without work."""
+    return rank == 0
+
+
+# ------------------------------------------------------------------------------------------------
 def run_reference(args):
     """Oracle arm: rank 0 only; each step = the oracle on a bounded row sample of the workload."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    if not reference_rank_runs(int(os.environ.get("RANK", "0"))):
         return
     import oracle
     from paper_2606_05933_b200 import workloads as wl, accounting as acc
@@ -222,13 +246,8 @@ def run_cuda(args):
     wall = time.perf_counter() - wall0
     clocks = sampler.stop()
     per_step_ms = np.array([e0.elapsed_time(e1) for e0, e1 in evs], dtype=np.float64)
-    total_ms = float(per_step_ms.sum())
-    if world > 1:
-        tt = torch.tensor([total_ms], dtype=torch.float64, device=devname)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
-    ms_per_step = total_ms / args.steps
-    value_us = ms_per_step * 1e3 / world           # replicas: N batches finish per step time
+    total_ms = max_over_ranks(float(per_step_ms.sum()), world, devname)
+    ms_per_step, value_us = replica_metric(total_ms, args.steps, world)
 
     # ---- dominant kernel: main attention launch, timed by events inside the library on the same stream ----
     h.set_kernel_timing(True)
@@ -278,10 +297,7 @@ def run_cuda(args):
         torch.cuda.synchronize()
     t2 = time.perf_counter()
     e2e_s = ((t1 - t0) - (t2 - t1)) / e2e_steps
-    if world > 1:
-        tt = torch.tensor([e2e_s], dtype=torch.float64, device=devname)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_s = float(tt.item())
+    e2e_s = max_over_ranks(e2e_s, world, devname)
     h2d = sum(x.numel() * x.element_size() for x in (hq, hk, hv, hbt, hqsl, hctx))
     d2h = hout.numel() * hout.element_size()
     assert torch.equal(hout, out.cpu()), "e2e output differs from the device-resident path"
