@@ -1,0 +1,78 @@
+"""SlidingChunker (§3.4, Algorithm 1) — host-side, CPU only."""
+import numpy as np
+
+from paper_2606_05933_b200.chunker import BatchForwarder, PrefillState, sliding_chunker, surface_predict_fn, window_bounds
+from paper_2606_05933_b200.features import features
+from paper_2606_05933_b200.predictor import BatchLatencyPredictor, load_surface
+
+
+def _toy_model(reqs):
+    """A latency model of the paper's form (Eq. 5): intercept + weights on Table 1's features."""
+    x = features(reqs)
+    return 8.0 + 2.5e-5 * x["x1"] + 0.12 * x["x4"] + 5e-4 * x["x5"] + 0.01 * x["x6"]
+
+
+def test_forward_allocates_in_sorted_order_and_respects_the_budget():
+    F = BatchForwarder(_toy_model, max_budget=512)
+    dec = [100, 2000, 30]
+    pre = [PrefillState(200, 0), PrefillState(1000, 64), PrefillState(50, 10)]
+    T, A = F.forward(dec, pre, 403)
+    assert A == [200, 200, 0] and sum(A) + len(dec) == 403
+    T2, A2 = F.forward(dec, pre, 10_000)                     # clamped to B = 512
+    assert sum(A2) + len(dec) == 512 and A2 == [200, 309, 0]
+    T0, A0 = F.forward(dec, pre, 0)                          # never below the decode tokens
+    assert A0 == [0, 0, 0] and T0 == _toy_model([(1, u) for u in dec])
+    assert T0 < T < T2
+
+
+def test_time_to_budget_is_the_largest_feasible_budget():
+    F = BatchForwarder(_toy_model, max_budget=2048)
+    dec = list(np.random.default_rng(0).integers(10, 4000, size=20))
+    pre = [PrefillState(1500, 0), PrefillState(3000, 500)]
+    for T in (1.0, 30.0, 45.0, 80.0, 1e9):
+        b = F.time_to_budget(dec, pre, T)
+        brute = [x for x in range(len(dec), F.B + 1) if F.pred(x, dec, pre) <= T]
+        assert b == (max(brute) if brute else len(dec))
+
+
+def test_window_bounds_eq_14_15():
+    t_cur, t_next = window_bounds([30.0, 12.0, 50.0], [40.0, 40.0, 25.0])
+    assert t_cur == 12.0 and t_next == min(30 - 12 + 40, 12 - 12 + 40, 50 - 12 + 25)
+
+
+def test_ternary_search_matches_brute_force_on_the_two_window_objective():
+    rng = np.random.default_rng(1)
+    for trial in range(20):
+        dec = list(rng.integers(10, 6000, size=int(rng.integers(1, 64))))
+        pre = [PrefillState(int(rng.integers(50, 4000)), int(rng.integers(0, 2000))) for _ in range(int(rng.integers(1, 5)))]
+        F = BatchForwarder(_toy_model, max_budget=int(rng.integers(256, 4096)))
+        t_cur, t_next = float(rng.uniform(15, 80)), float(rng.uniform(15, 120))
+        b_star, a_star, t_star, b_sigma = sliding_chunker(F, dec, pre, t_cur, t_next)
+        assert len(dec) <= b_star <= F.B and sum(a_star) <= b_star - len(dec)
+        two = lambda b: F.pred(b, dec, pre) + F.pred(b_sigma - b, dec, pre)
+        assert abs(t_star - two(b_star)) < 1e-9
+        # Algorithm 1 evaluates {l0, r0, mid of the final bracket}: never worse than both ends of the range, and within
+        # the final bracket's resolution of the exhaustive optimum of the (here unimodal-or-flat) objective
+        best = min(two(b) for b in range(len(dec), F.B + 1))
+        assert t_star <= min(two(len(dec)), two(F.B)) + 1e-9
+        assert t_star - best <= 0.02 * best + 0.5
+
+
+def test_chunker_on_the_measured_surface():
+    """End to end with the predictor fitted on the committed B200 latency surface.  The unconstrained least-squares fit
+    on this small grid is not monotone in the budget (negative weights on x6 / x7), so only what Algorithm 1 guarantees
+    is asserted: a budget in [|D|, B], an allocation that spends it in sorted order, T* = the two-window objective at
+    B*, and B* no worse than the two ends of the range."""
+    rows, X, y, scenes, shapes = load_surface("profiles/r1_v4_surface.csv")
+    keep = [i for i, s in enumerate(shapes) if s == "32/8/128"]
+    p = BatchLatencyPredictor().fit(X[keep], y[keep], [scenes[i] for i in keep])
+    F = BatchForwarder(surface_predict_fn(p), max_budget=2048)
+    dec = list(np.random.default_rng(2).integers(200, 6000, size=64))
+    pre = [PrefillState(1800, 0), PrefillState(900, 1024)]
+    for slack in (140.0, 180.0, 250.0, 400.0):
+        b_star, a_star, t_star, b_sigma = sliding_chunker(F, dec, pre, slack, slack + 100.0)
+        assert len(dec) <= b_star <= F.B
+        assert sum(a_star) == min(b_star - len(dec), 2700) and a_star[0] == min(1800, b_star - len(dec))
+        two = lambda b: F.pred(b, dec, pre) + F.pred(b_sigma - b, dec, pre)
+        assert abs(t_star - two(b_star)) < 1e-9
+        assert t_star <= min(two(len(dec)), two(F.B)) + 1e-9
