@@ -8,7 +8,7 @@ samples; inference uses the expert if one exists, else the global model (PAPER.m
 threshold but gives no value: 12 here (reading 15).  Fit = ordinary least squares (the paper says
 "lightweight ... linear"; no regulariser is mentioned), features scaled to unit max for conditioning only.
 
-    python -m paper_2606_05933_b200.predictor profiles/r1_v4_surface.csv
+    python -m paper_2606_05933_b200.predictor profiles/r1_v4_surface.csv profiles/r1_v4_surface_dense.csv
 
 prints MAE / RMSE / R^2 the way Table 5 does, in-sample and leave-one-out.
 """
@@ -84,8 +84,10 @@ def scores(y: np.ndarray, yhat: np.ndarray) -> Dict[str, float]:
             "r2": 1.0 - ss_res / ss_tot if ss_tot > 0 else float("nan")}
 
 
-def load_surface(path: str):
-    rows = list(csv.DictReader(open(path)))
+def load_surface(path):
+    """One CSV path, or several (grid + dense points) to be concatenated."""
+    paths = [path] if isinstance(path, str) else list(path)
+    rows = [r for p in paths for r in csv.DictReader(open(p))]
     X = np.array([[float(r[f]) for f in FEATURES] for r in rows])
     y = np.array([float(r["median_us"]) for r in rows])
     scenes = [r["scene"] for r in rows]
@@ -116,7 +118,7 @@ def evaluate(path: str, shape: str = "32/8/128", min_expert_samples: int = 12) -
 
 def main(argv: Optional[List[str]] = None):
     argv = sys.argv[1:] if argv is None else argv
-    path = argv[0] if argv else "profiles/r1_v4_surface.csv"
+    path = argv if argv else ["profiles/r1_v4_surface.csv", "profiles/r1_v4_surface_dense.csv"]
     res = evaluate(path)
     print(f"surface: {path}  points (8B shape): {res['n']}")
     print(f"experts trained for: {sorted(res['experts'])}")

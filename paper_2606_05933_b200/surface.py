@@ -30,8 +30,22 @@ FIELDS = ["point", "name", "seed", "shape", "scene", "R", "T", "chunk", "n_prefi
           "median_us", "p10_us", "p90_us", "frac_of_roofline", "prefill_only_us", "decode_only_us", "overlap"]
 
 
-def surface_points(with_c4: bool = False) -> List[tuple]:
+def dense_points() -> List[tuple]:
+    """Extra points between the grid lines (for the predictor fit): more chunk budgets and decode counts."""
+    pts = []
+    for nd in (0, 16, 48, 64, 96, 192):
+        for C in (0, 128, 384, 768, 1536, 2048):
+            for n in (1, 2):
+                if (C == 0 and (nd == 0 or n == 2)):
+                    continue
+                pts.append((f"DN:{C},{n},{nd}", lambda C=C, n=n, nd=nd: wl.config_dense(C, n, nd)))
+    return pts
+
+
+def surface_points(with_c4: bool = False, dense: bool = False) -> List[tuple]:
     """(point id, Batch factory) for the whole grid, in a fixed order."""
+    if dense:
+        return dense_points()
     pts = []
     for nd in (32, 128):                                   # BASELINE.json configs[2]: the predictor grid
         for C in (256, 512, 1024, 2048):
@@ -97,6 +111,7 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--with-c4", action="store_true", help="include the 40 GB-pool decode-heavy config")
     ap.add_argument("--only", default=None, help="comma-separated point-id prefixes")
+    ap.add_argument("--dense", action="store_true", help="the extra between-the-lines points instead of the grid")
     args = ap.parse_args(argv)
     import torch
     if not torch.cuda.is_available():
@@ -108,7 +123,7 @@ def main(argv=None):
     with open(args.out, "w", newline="") as f:
         wr = csv.DictWriter(f, fieldnames=FIELDS)
         wr.writeheader()
-        for pid, make in surface_points(args.with_c4):
+        for pid, make in surface_points(args.with_c4, args.dense):
             if args.only and not any(pid.startswith(p) for p in args.only.split(",")):
                 continue
             b = make()

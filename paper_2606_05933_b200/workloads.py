@@ -143,6 +143,18 @@ def config_c3(C: int, n: int, N_d: int, ctx_median: int = 1500, shuffle: bool = 
                             "ctx_median": ctx_median})
 
 
+def config_dense(C: int, n: int, N_d: int, ctx_median: int = 1500) -> Batch:
+    """Extra points of the latency surface between the C3 grid lines (same recipe as config_c3, own seeds): any chunk
+    budget C >= 0 over n prefill requests (ctx U{0..4096}) + N_d >= 0 decodes (ctx lognormal, cap 8192)."""
+    seed = 500000 + 17 * C + 1009 * n + 31 * N_d + 7 * ctx_median
+    rng = np.random.default_rng(seed)
+    pu = rng.integers(0, 4096, size=max(n, 1), endpoint=True)
+    du = _lognormal_ctx(rng, ctx_median, N_d, 8192) if N_d > 0 else np.zeros(0, dtype=np.int64)
+    reqs = ([(c, int(u)) for c, u in zip(c3_split(C, n), pu) if c > 0] if C > 0 else []) + [(1, int(u)) for u in du]
+    return make_batch(f"DN-C{C}-n{n}-Nd{N_d}-m{ctx_median}", 32, 8, 128, reqs, seed, rng=rng,
+                      meta={"chunk": C, "n_prefill": n if C > 0 else 0, "n_decode": N_d, "ctx_median": ctx_median})
+
+
 def config_c4(seed: int = 4, num_requests: int = 256, pool_pages: int = 610352) -> Batch:
     """C4: 256 decodes, ctx U{1024..16384}, pages scattered over a 2 x 20 GB pool."""
     rng = np.random.default_rng(seed)
