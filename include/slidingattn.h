@@ -26,8 +26,19 @@
  *     Query head h uses KV head h / (num_q_heads/num_kv_heads).
  *   - Slots past u_r+c_r in a last page, pages in no block table and block-table tail entries may
  *     hold ANY bit pattern; they never influence results and are never written.
- *   - Device-resident metadata cannot be validated without a sync: page ids >= num_pages, a
- *     non-monotone query_start_loc or ceil((u_r+c_r)/16) > max_pages_per_req are undefined behaviour.
+ *   - Device-resident metadata cannot be validated on the host without a sync.  Without
+ *     SS_FLAG_DEBUG_CHECKS, page ids outside [0, num_pages), a query_start_loc that is not
+ *     0 = qsl[0] <= ... <= qsl[R] = T, a negative ctx_len or ceil((u_r+c_r)/16) > max_pages_per_req are
+ *     undefined behaviour.  With the flag, every ss_kv_append / ss_mixed_attention first runs a device-side
+ *     check of exactly these conditions; on a violation it records (code, request, value) in a device flag
+ *     and the call - and every later call on the handle - touches neither the caches nor `out` until
+ *     ss_poll_device_error has reported and cleared it.
+ *   - ONE CALL IN FLIGHT PER HANDLE: the work-queue tickets and split-arrival counters are handle-owned
+ *     device memory that the kernels re-arm themselves, so all calls on one handle must be ordered on one
+ *     stream (or by events).  Use one handle per stream for concurrency.  If a launch was aborted
+ *     (sticky CUDA error, device reset), call ss_reset before reusing the handle.
+ *   - scale must be finite and > 0 (SS_ERR_INVALID_ARG otherwise): the kernels fold log2(e) into it and
+ *     take the running maximum of the raw scores, which is the maximum of the scaled scores only for scale > 0.
  */
 #ifndef SLIDINGATTN_H
 #define SLIDINGATTN_H
@@ -39,7 +50,7 @@
 extern "C" {
 #endif
 
-#define SS_VERSION 100
+#define SS_VERSION 200
 
 typedef enum ss_status {
     SS_OK = 0,
@@ -47,8 +58,12 @@ typedef enum ss_status {
     SS_ERR_WORKSPACE_TOO_SMALL = -2,
     SS_ERR_UNSUPPORTED_DEVICE = -3,  /* current device is not compute capability 10.x */
     SS_ERR_CUDA = -4,                /* a CUDA runtime/driver call failed; see ss_last_error_string */
-    SS_ERR_NOT_IMPLEMENTED = -5
+    SS_ERR_NOT_IMPLEMENTED = -5,
+    SS_ERR_DEVICE_CHECK = -6         /* ss_poll_device_error: the in-kernel metadata check (SS_FLAG_DEBUG_CHECKS) tripped */
 } ss_status;
+
+/* ss_config.flags */
+#define SS_FLAG_DEBUG_CHECKS 1u      /* "debug build" of SURVEY.md section 8(b): bounds-check device metadata in-kernel */
 
 typedef struct ss_handle ss_handle;  /* opaque; owns tensor maps, SM count, small staging buffers */
 
@@ -61,27 +76,8 @@ typedef struct ss_config {
     int32_t max_requests;       /* upper bound on R */
     int32_t max_tokens;         /* upper bound on T */
     int32_t max_pages_per_req;  /* second dimension of block_table */
+    uint32_t flags;             /* 0 or SS_FLAG_DEBUG_CHECKS */
 } ss_config;
-
-/* One entry of the device work list (a2); exposed so tests can check the builder.
- * kind 1 = prefill tile: query rows [row0, row0+nrows) of request req (c_r > 1, Eq. 2),
- *          query head `head`, keys [0, kv_end);
- * kind 2 = decode split: the single row of request req (c_r == 1), KV head `head`, keys
- *          [kv_begin, kv_end); partial results go to slot `partial` unless nsplit == 1. */
-typedef struct ss_work_item {
-    int32_t kind;
-    int32_t req;
-    int32_t head;
-    int32_t row0;       /* flat row index into q/out */
-    int32_t nrows;
-    int32_t kv_begin;
-    int32_t kv_end;
-    int32_t split;      /* index of this split, 0 <= split < nsplit */
-    int32_t nsplit;
-    int32_t partial;    /* decode: first partial slot of this (req, kv head), slot = partial + split */
-    int32_t q_pos0;     /* prefill: chunk-relative index j of the first row (row j sees keys 0..u+j) */
-    int32_t reserved;
-} ss_work_item;
 
 /* Lifetime.  ss_create binds the handle to the two cache tensors (TMA descriptors are encoded once)
  * and to the current CUDA device.  The caches stay caller-owned and must outlive the handle. */
@@ -111,6 +107,7 @@ int ss_kv_append(ss_handle* h, const void* k_new, const void* v_new, const int32
  * must already hold the u_r + c_r tokens (run ss_kv_append for the same batch earlier on the same
  * stream).  Requests with c_r == 1 take the split-KV decode path, c_r > 1 the tensor-core chunk path,
  * c_r == 0 contributes nothing; any mix and any request order is served by one call.
+ * scale: finite and > 0, else SS_ERR_INVALID_ARG (benchmarks pass 1/sqrt(head_dim)).
  * lse_or_null: optional [T][Hq] fp32 log-sum-exp (natural log) of the scaled scores, a test aid.
  * workspace: device memory of at least ss_workspace_bytes(h), contents undefined in/out.
  * Bitwise reproducible run to run for identical inputs.  All pointers device.
@@ -119,15 +116,6 @@ int ss_mixed_attention(ss_handle* h, const void* q, const int32_t* block_table,
                        const int32_t* query_start_loc, const int32_t* ctx_lens, int32_t R, int32_t T,
                        float scale, void* out, float* lse_or_null, void* workspace,
                        size_t workspace_bytes, void* cuda_stream);
-
-/*
- * a2 alone (test aid): build the work list for a batch into `workspace` exactly as ss_mixed_attention
- * does, then copy it to the host (this call DOES synchronise the stream).  items_host may be NULL to
- * query counts only.  counts_host[0] = number of prefill items, [1] = decode items, [2] = partial slots.
- */
-int ss_build_worklist(ss_handle* h, const int32_t* query_start_loc, const int32_t* ctx_lens, int32_t R,
-                      int32_t T, void* workspace, size_t workspace_bytes, ss_work_item* items_host,
-                      int32_t max_items, int32_t counts_host[3], void* cuda_stream);
 
 /*
  * End-to-end iteration from HOST buffers (what a serving loop without device-resident activations
@@ -140,37 +128,20 @@ int ss_iteration_host(ss_handle* h, const void* q_host, const void* k_new_host, 
                       const int32_t* ctx_lens_host, int32_t R, int32_t T, float scale, void* out_host,
                       void* cuda_stream);
 
-/* Which kernels the last ss_mixed_attention / ss_kv_append on this handle launched (count), so a
- * caller can report launches per iteration without a profiler. */
-int ss_last_launch_count(const ss_handle* h);
+/*
+ * Debug-check report.  Synchronises `cuda_stream`, reads the device error flag and
+ * clears it.  SS_OK if no check tripped (always, when the handle was created without SS_FLAG_DEBUG_CHECKS);
+ * SS_ERR_DEVICE_CHECK otherwise, with ss_last_error_string naming the violated condition, the request index
+ * and the offending value.  Calls issued between the violation and this poll did nothing.
+ */
+int ss_poll_device_error(ss_handle* h, void* cuda_stream);
 
-/* Measurement aid: when on, ss_mixed_attention brackets its dominant kernel(s) (a3+a4 main launch) with
- * CUDA events on the caller's stream; ss_last_kernel_time_us then synchronises on them and returns the
- * device time of the last call's main launch in microseconds (SS_ERR_INVALID_ARG if timing was off). */
-int ss_set_kernel_timing(ss_handle* h, int on);
-int ss_last_kernel_time_us(ss_handle* h, float* main_us);
-
-/* Debug: force the plain one-warp-per-row CUDA kernel (no tensor cores) for every row. 0 = off. */
-int ss_debug_force_simple_path(ss_handle* h, int on);
-
-/* Debug / tuning knobs; value 0 restores the automatic choice.  which: 1 = CTAs of the main launch (default one
- * per SM), 2 = number of CTAs that drain the decode queue first (default: balanced from the batch's decode bytes and
- * prefill flops by the planner; -1 = none), 3 = decode split length in keys (multiple of 128), 4 = nonzero forces the
- * two-launch route (stand-alone work-list kernel + main kernel reading its items) that batches of more than 256
- * requests take; by default smaller batches are planned inside the main kernel (one launch).
- * Results never depend on these; only timing does.  SS_ERR_INVALID_ARG for an unknown key. */
-int ss_debug_set_param(ss_handle* h, int which, int value);
-
-/* Measurement aid: per-CTA timeline of the main launch.  `trace_dev` is a DEVICE buffer of
- * num_ctas * words_per_cta uint64 words (caller-owned; NULL switches tracing off; words_per_cta >= 6).  Per CTA the
- * kernel writes word 0 = %globaltimer at entry (ns), 1 = after setup + grid dependency wait, 2 = worker warps' exit,
- * 3 = item count, 4 = exit of the MMA / split-merge warp, 5 = unused, then 9 words per item while they fit: start ns,
- * end ns, kind << 32 | KV tiles, first tile ready ns, tile loop end ns, and 4 epilogue stamps (decode items only).
- * Results never depend on it. */
-int ss_debug_set_trace(ss_handle* h, void* trace_dev, int32_t words_per_cta);
+/* Re-zero the handle-owned device state (queue tickets, split-arrival counters, error flag) on `cuda_stream`.
+ * Only needed after a launch on this handle was aborted mid-flight. */
+int ss_reset(ss_handle* h, void* cuda_stream);
 
 const char* ss_status_string(int status);
-const char* ss_last_error_string(const ss_handle* h);   /* detail of the last SS_ERR_CUDA on this handle */
+const char* ss_last_error_string(const ss_handle* h);   /* detail of the last SS_ERR_CUDA / SS_ERR_DEVICE_CHECK on this handle */
 int ss_version(void);
 
 #ifdef __cplusplus

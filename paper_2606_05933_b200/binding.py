@@ -15,17 +15,24 @@ LIB_PATH = _PKG / "libslidingattn.so"
 _lib = None
 
 SS_OK = 0
+SS_ERR_INVALID_ARG = -1
+SS_ERR_DEVICE_CHECK = -6
+SS_FLAG_DEBUG_CHECKS = 1
+# include/slidingattn.h (the product boundary) ...
 EXPORTS = ["ss_version", "ss_status_string", "ss_last_error_string", "ss_create", "ss_destroy",
-           "ss_workspace_bytes", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
-           "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path",
-           "ss_debug_set_param", "ss_debug_set_trace", "ss_set_kernel_timing", "ss_last_kernel_time_us"]
+           "ss_workspace_bytes", "ss_kv_append", "ss_mixed_attention", "ss_iteration_host",
+           "ss_poll_device_error", "ss_reset"]
+# ... and include/slidingattn_debug.h (test / tuning / measurement aids)
+DEBUG_EXPORTS = ["ss_build_worklist", "ss_last_launch_count", "ss_debug_force_simple_path",
+                 "ss_debug_set_param", "ss_debug_set_trace", "ss_set_kernel_timing", "ss_last_kernel_time_us"]
 
 
 class ss_config(ctypes.Structure):
     _fields_ = [("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32),
                 ("head_dim", ctypes.c_int32), ("page_size", ctypes.c_int32),
                 ("num_pages", ctypes.c_int64), ("max_requests", ctypes.c_int32),
-                ("max_tokens", ctypes.c_int32), ("max_pages_per_req", ctypes.c_int32)]
+                ("max_tokens", ctypes.c_int32), ("max_pages_per_req", ctypes.c_int32),
+                ("flags", ctypes.c_uint32)]
 
 
 class ss_work_item(ctypes.Structure):
@@ -66,21 +73,37 @@ def load():
                                       ctypes.POINTER(i32 * 3), vp]
     lib.ss_iteration_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
     lib.ss_last_launch_count.argtypes = [vp]
+    lib.ss_poll_device_error.argtypes = [vp, vp]
+    lib.ss_reset.argtypes = [vp, vp]
     lib.ss_debug_force_simple_path.argtypes = [vp, ctypes.c_int]
     lib.ss_debug_set_param.argtypes = [vp, ctypes.c_int, ctypes.c_int]
     lib.ss_debug_set_trace.argtypes = [vp, vp, i32]
     lib.ss_set_kernel_timing.argtypes = [vp, ctypes.c_int]
     lib.ss_last_kernel_time_us.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
-    for name in ("ss_create", "ss_destroy", "ss_kv_append", "ss_mixed_attention", "ss_build_worklist",
-                 "ss_iteration_host", "ss_last_launch_count", "ss_debug_force_simple_path",
-                 "ss_debug_set_param", "ss_debug_set_trace", "ss_set_kernel_timing", "ss_last_kernel_time_us"):
-        getattr(lib, name).restype = ctypes.c_int
+    for name in EXPORTS + DEBUG_EXPORTS:
+        if name not in ("ss_status_string", "ss_last_error_string", "ss_workspace_bytes"):
+            getattr(lib, name).restype = ctypes.c_int
     _lib = lib
     return lib
 
 
 def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
     return None if t is None else t.data_ptr()
+
+
+def _want(t: torch.Tensor, name: str, dtype, cuda: bool = True, shape=None):
+    """The C ABI takes raw pointers: a wrong dtype (torch's default int64 indices!), a strided view or a host
+    tensor would be read as garbage with no error, so refuse them here."""
+    if not isinstance(t, torch.Tensor):
+        raise SlidingAttnError(f"{name}: expected a torch.Tensor")
+    if t.dtype != dtype:
+        raise SlidingAttnError(f"{name}: expected {dtype}, got {t.dtype}")
+    if cuda != t.is_cuda:
+        raise SlidingAttnError(f"{name}: expected a {'CUDA' if cuda else 'host'} tensor")
+    if not t.is_contiguous():
+        raise SlidingAttnError(f"{name}: must be contiguous")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise SlidingAttnError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
 
 
 def _stream_ptr(stream) -> Optional[int]:
@@ -93,7 +116,8 @@ class SlidingAttn:
     """Handle bound to one pair of paged caches [num_pages, Hkv, 16, D] bf16 on the current device."""
 
     def __init__(self, num_q_heads: int, num_kv_heads: int, head_dim: int, k_cache: torch.Tensor,
-                 v_cache: torch.Tensor, max_requests: int, max_tokens: int, max_pages_per_req: int):
+                 v_cache: torch.Tensor, max_requests: int, max_tokens: int, max_pages_per_req: int,
+                 debug_checks: bool = False):
         self.lib = load()
         if not (k_cache.is_cuda and v_cache.is_cuda):
             raise SlidingAttnError("caches must be CUDA tensors (no CPU path exists)")
@@ -101,7 +125,7 @@ class SlidingAttn:
         P, Hkv, page, D = k_cache.shape
         assert Hkv == num_kv_heads and D == head_dim
         self.cfg = ss_config(num_q_heads, num_kv_heads, head_dim, page, P, max_requests, max_tokens,
-                             max_pages_per_req)
+                             max_pages_per_req, SS_FLAG_DEBUG_CHECKS if debug_checks else 0)
         self.k_cache, self.v_cache = k_cache, v_cache
         self._h = ctypes.c_void_p()
         self._check(self.lib.ss_create(ctypes.byref(self._h), ctypes.byref(self.cfg), k_cache.data_ptr(),
@@ -112,7 +136,9 @@ class SlidingAttn:
     def _check(self, rc: int, create: bool = False):
         if rc != SS_OK:
             detail = b"" if create or not self._h else self.lib.ss_last_error_string(self._h)
-            raise SlidingAttnError(f"{self.lib.ss_status_string(rc).decode()} ({rc}) {detail.decode()}")
+            err = SlidingAttnError(f"{self.lib.ss_status_string(rc).decode()} ({rc}) {detail.decode()}")
+            err.status = rc
+            raise err
 
     def close(self):
         if getattr(self, "_h", None):
@@ -126,16 +152,33 @@ class SlidingAttn:
             pass
 
     # ---- the two calls of the path -------------------------------------------------------------
+    def _check_batch(self, block_table, query_start_loc, ctx_lens, cuda=True):
+        R = ctx_lens.shape[0]
+        _want(ctx_lens, "ctx_lens", torch.int32, cuda, (R,))
+        _want(query_start_loc, "query_start_loc", torch.int32, cuda, (R + 1,))
+        _want(block_table, "block_table", torch.int32, cuda, (R, self.cfg.max_pages_per_req))
+        return R
+
     def kv_append(self, k_new, v_new, block_table, query_start_loc, ctx_lens, stream=None):
-        R, T = ctx_lens.shape[0], k_new.shape[0]
+        R, T = self._check_batch(block_table, query_start_loc, ctx_lens), k_new.shape[0]
+        kv_shape = (T, self.cfg.num_kv_heads, self.cfg.head_dim)
+        _want(k_new, "k_new", torch.bfloat16, True, kv_shape)
+        _want(v_new, "v_new", torch.bfloat16, True, kv_shape)
         self._check(self.lib.ss_kv_append(self._h, _ptr(k_new), _ptr(v_new), _ptr(block_table),
                                           _ptr(query_start_loc), _ptr(ctx_lens), R, T, _stream_ptr(stream)))
 
     def mixed_attention(self, q, block_table, query_start_loc, ctx_lens, scale, out=None, lse=None,
                         stream=None):
-        R, T = ctx_lens.shape[0], q.shape[0]
+        R, T = self._check_batch(block_table, query_start_loc, ctx_lens), q.shape[0]
+        q_shape = (T, self.cfg.num_q_heads, self.cfg.head_dim)
+        _want(q, "q", torch.bfloat16, True, q_shape)
         if out is None:
             out = torch.empty_like(q)
+        _want(out, "out", torch.bfloat16, True, q_shape)
+        if lse is not None:
+            _want(lse, "lse", torch.float32, True)
+            if lse.numel() < T * self.cfg.num_q_heads:
+                raise SlidingAttnError("lse: needs at least T * Hq elements")
         self._check(self.lib.ss_mixed_attention(self._h, _ptr(q), _ptr(block_table), _ptr(query_start_loc),
                                                 _ptr(ctx_lens), R, T, float(scale), _ptr(out), _ptr(lse),
                                                 self.workspace.data_ptr(), self.workspace_bytes,
@@ -161,11 +204,23 @@ class SlidingAttn:
 
     def iteration_host(self, q, k_new, v_new, block_table, query_start_loc, ctx_lens, scale, out, stream=None):
         """Host (pinned) tensors in, host tensor out; H2D + append + attention + D2H + sync inside."""
-        R, T = ctx_lens.shape[0], q.shape[0]
+        R, T = self._check_batch(block_table, query_start_loc, ctx_lens, cuda=False), q.shape[0]
+        _want(q, "q", torch.bfloat16, False, (T, self.cfg.num_q_heads, self.cfg.head_dim))
+        _want(out, "out", torch.bfloat16, False, (T, self.cfg.num_q_heads, self.cfg.head_dim))
+        for name, x in (("k_new", k_new), ("v_new", v_new)):
+            if x is not None:
+                _want(x, name, torch.bfloat16, False, (T, self.cfg.num_kv_heads, self.cfg.head_dim))
         self._check(self.lib.ss_iteration_host(self._h, _ptr(q), _ptr(k_new), _ptr(v_new), _ptr(block_table),
                                                _ptr(query_start_loc), _ptr(ctx_lens), R, T, float(scale),
                                                _ptr(out), _stream_ptr(stream)))
         return out
+
+    def poll_device_error(self, stream=None) -> None:
+        """Synchronises; raises SlidingAttnError(SS_ERR_DEVICE_CHECK ...) if a debug check tripped since the last poll."""
+        self._check(self.lib.ss_poll_device_error(self._h, _stream_ptr(stream)))
+
+    def reset(self, stream=None) -> None:
+        self._check(self.lib.ss_reset(self._h, _stream_ptr(stream)))
 
     def last_launch_count(self) -> int:
         return int(self.lib.ss_last_launch_count(self._h))
@@ -204,8 +259,8 @@ def mixed_attention(handle: SlidingAttn, q, block_table, query_start_loc, ctx_le
     return handle.mixed_attention(q, block_table, query_start_loc, ctx_lens, scale, out, lse, stream)
 
 
-def handle_for(batch, tensors, extra_tokens: int = 0) -> SlidingAttn:
+def handle_for(batch, tensors, extra_tokens: int = 0, debug_checks: bool = False) -> SlidingAttn:
     """Convenience: a handle sized for one workloads.Batch."""
     return SlidingAttn(batch.num_q_heads, batch.num_kv_heads, batch.head_dim, tensors.k_cache, tensors.v_cache,
                        max_requests=max(batch.R, 1), max_tokens=max(batch.T + extra_tokens, 1),
-                       max_pages_per_req=batch.max_pages_per_req)
+                       max_pages_per_req=batch.max_pages_per_req, debug_checks=debug_checks)

@@ -1,5 +1,6 @@
 // C ABI of libslidingattn (include/slidingattn.h): argument checks, handle, launch sequencing.
 // No arithmetic of the method lives here; every step of the path runs in the kernels.
+#include <math.h>
 #include <new>
 #include <string.h>
 
@@ -85,6 +86,7 @@ const char* ss_status_string(int s) {
         case SS_ERR_UNSUPPORTED_DEVICE: return "SS_ERR_UNSUPPORTED_DEVICE";
         case SS_ERR_CUDA: return "SS_ERR_CUDA";
         case SS_ERR_NOT_IMPLEMENTED: return "SS_ERR_NOT_IMPLEMENTED";
+        case SS_ERR_DEVICE_CHECK: return "SS_ERR_DEVICE_CHECK";
         default: return "SS_ERR_UNKNOWN";
     }
 }
@@ -106,6 +108,8 @@ int ss_create(ss_handle** out_handle, const ss_config* cfg, void* k_cache, void*
         cfg->max_pages_per_req <= 0)
         return SS_ERR_INVALID_ARG;
     if ((int64_t)cfg->max_pages_per_req * kPage > (int64_t)1 << 30) return SS_ERR_INVALID_ARG;
+    if (cfg->flags & ~(uint32_t)SS_FLAG_DEBUG_CHECKS) return SS_ERR_INVALID_ARG;
+    if (!workspace_layout(*cfg, 256).ok) return SS_ERR_INVALID_ARG;   // worst-case item count must fit the int32 index space
 
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return SS_ERR_CUDA;
@@ -122,7 +126,16 @@ int ss_create(ss_handle** out_handle, const ss_config* cfg, void* k_cache, void*
     h->group = cfg->num_q_heads / cfg->num_kv_heads;
     h->k_cache = k_cache;
     h->v_cache = v_cache;
+    h->debug_checks = (cfg->flags & SS_FLAG_DEBUG_CHECKS) ? 1 : 0;
     h->ws = workspace_layout(h->cfg, h->num_sms);
+    if (!h->ws.ok) {                 // worst-case item count of this config overflows the int32 index space
+        delete h;
+        return SS_ERR_INVALID_ARG;
+    }
+    if (init_main_attention(cfg->head_dim) != cudaSuccess) {
+        delete h;
+        return SS_ERR_CUDA;
+    }
     int rc = encode_cache_map(h, &h->tmap_k, k_cache);
     if (rc == SS_OK) rc = encode_cache_map(h, &h->tmap_v, v_cache);
     if (rc != SS_OK) {
@@ -130,7 +143,8 @@ int ss_create(ss_handle** out_handle, const ss_config* cfg, void* k_cache, void*
         return rc;
     }
     h->have_tmaps = true;
-    const size_t state_bytes = sizeof(int32_t) * (4 + (size_t)cfg->max_requests * cfg->num_kv_heads);
+    const size_t state_bytes = sizeof(int32_t) * ((size_t)kStateCounters + (size_t)cfg->max_requests * cfg->num_kv_heads);
+    h->state_bytes = state_bytes;
     if (cudaMalloc((void**)&h->state, state_bytes) != cudaSuccess || cudaMemset(h->state, 0, state_bytes) != cudaSuccess) {
         if (h->state) cudaFree(h->state);
         delete h;
@@ -195,6 +209,12 @@ int ss_debug_force_simple_path(ss_handle* hh, int on) {
 int ss_debug_set_param(ss_handle* hh, int which, int value) {
     Handle* h = (Handle*)hh;
     if (!h || which < 1 || which >= 8) return SS_ERR_INVALID_ARG;
+    if (which == kDbgSplitKeys && value > 0) {
+        // the workspace's partial slots are sized for split lengths in [kMinSplitKeys, kMaxSplitKeys]
+        value = (value + kTileKeys - 1) / kTileKeys * kTileKeys;
+        if (value < kMinSplitKeys) value = kMinSplitKeys;
+        if (value > kMaxSplitKeys) value = kMaxSplitKeys;
+    }
     h->dbg[which] = value;
     return SS_OK;
 }
@@ -215,9 +235,11 @@ int ss_kv_append(ss_handle* hh, const void* k_new, const void* v_new, const int3
     h->last_launches = 0;
     if (R == 0 || T == 0) return SS_OK;
     if (!block_table || (((uintptr_t)block_table) & 3u)) return SS_ERR_INVALID_ARG;
+    if (h->debug_checks)
+        SS_CUDA(h, launch_validate(h, block_table, query_start_loc, ctx_lens, R, T, (cudaStream_t)cuda_stream), "validate launch");
     SS_CUDA(h, launch_kv_append(h, k_new, v_new, block_table, query_start_loc, ctx_lens, R, T, (cudaStream_t)cuda_stream),
             "kv_append launch");
-    h->last_launches = 1;
+    h->last_launches = 1 + h->debug_checks;
     return SS_OK;
 }
 
@@ -233,7 +255,9 @@ int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table,
     if (lse_or_null && (((uintptr_t)lse_or_null) & 3u)) return SS_ERR_INVALID_ARG;
     if (!workspace || !aligned16(workspace)) return SS_ERR_INVALID_ARG;
     if (workspace_bytes < h->ws.total) return SS_ERR_WORKSPACE_TOO_SMALL;
+    if (!(scale > 0.f) || !isfinite(scale)) return SS_ERR_INVALID_ARG;      // see slidingattn.h: running max of raw scores
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (h->debug_checks) SS_CUDA(h, launch_validate(h, block_table, query_start_loc, ctx_lens, R, T, st), "validate launch");
 
     if (h->force_simple) {
         SS_CUDA(h, launch_simple_attention(h, q, block_table, query_start_loc, ctx_lens, R, T, scale, out, lse_or_null, st),
@@ -252,8 +276,34 @@ int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table,
         SS_CUDA(h, cudaEventRecord(h->ev1, st), "timing event");
         h->timing_valid = 1;
     }
-    h->last_launches = (two_kernels ? 1 : 0) + n;
+    h->last_launches = (two_kernels ? 1 : 0) + n + h->debug_checks;
     return SS_OK;
+}
+
+int ss_reset(ss_handle* hh, void* cuda_stream) {
+    Handle* h = (Handle*)hh;
+    if (!h) return SS_ERR_INVALID_ARG;
+    SS_CUDA(h, cudaMemsetAsync(h->state, 0, h->state_bytes, (cudaStream_t)cuda_stream), "state reset");
+    return SS_OK;
+}
+
+int ss_poll_device_error(ss_handle* hh, void* cuda_stream) {
+    Handle* h = (Handle*)hh;
+    if (!h) return SS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int32_t rec[4] = {0, 0, 0, 0};
+    SS_CUDA(h, cudaMemcpyAsync(rec, h->state + kStateErr, sizeof rec, cudaMemcpyDeviceToHost, st), "error flag copy");
+    SS_CUDA(h, cudaStreamSynchronize(st), "error flag sync");
+    if (rec[0] == 0) return SS_OK;
+    SS_CUDA(h, cudaMemsetAsync(h->state + kStateErr, 0, sizeof rec, st), "error flag clear");
+    SS_CUDA(h, cudaStreamSynchronize(st), "error flag sync");
+    const char* what = rec[0] == kChkQsl            ? "query_start_loc is not 0 = qsl[0] <= ... <= qsl[R] = T"
+                       : rec[0] == kChkCtxNegative  ? "negative ctx_len"
+                       : rec[0] == kChkTooManyPages ? "ceil((u+c)/16) exceeds max_pages_per_req"
+                       : rec[0] == kChkPageId       ? "block_table page id outside [0, num_pages)"
+                                                    : "unknown check";
+    snprintf(h->err, sizeof h->err, "device check %d: %s (request %d, value %d, limit %d)", rec[0], what, rec[1], rec[2], rec[3]);
+    return SS_ERR_DEVICE_CHECK;
 }
 
 int ss_build_worklist(ss_handle* hh, const int32_t* query_start_loc, const int32_t* ctx_lens, int32_t R, int32_t T,
@@ -299,15 +349,22 @@ int ss_iteration_host(ss_handle* hh, const void* q_host, const void* k_new_host,
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t q_max = (size_t)c.max_tokens * c.num_q_heads * c.head_dim * 2;
     const size_t kv_max = (size_t)c.max_tokens * c.num_kv_heads * c.head_dim * 2;
-    if (!h->st_q) {
-        SS_CUDA(h, cudaMalloc(&h->st_q, q_max), "staging alloc");
-        SS_CUDA(h, cudaMalloc(&h->st_out, q_max), "staging alloc");
-        SS_CUDA(h, cudaMalloc(&h->st_knew, kv_max), "staging alloc");
-        SS_CUDA(h, cudaMalloc(&h->st_vnew, kv_max), "staging alloc");
-        SS_CUDA(h, cudaMalloc(&h->st_ws, h->ws.total), "staging alloc");
-        SS_CUDA(h, cudaMalloc((void**)&h->st_bt, sizeof(int32_t) * (size_t)c.max_requests * c.max_pages_per_req), "staging alloc");
-        SS_CUDA(h, cudaMalloc((void**)&h->st_qsl, sizeof(int32_t) * (size_t)(c.max_requests + 1)), "staging alloc");
-        SS_CUDA(h, cudaMalloc((void**)&h->st_ctx, sizeof(int32_t) * (size_t)c.max_requests), "staging alloc");
+    if (!h->st_ctx) {
+        // all or nothing: st_ctx (allocated last) doubles as the "staging ready" mark
+        void** slots[] = {&h->st_q, &h->st_out, &h->st_knew, &h->st_vnew, &h->st_ws, (void**)&h->st_bt, (void**)&h->st_qsl,
+                          (void**)&h->st_ctx};
+        const size_t sizes[] = {q_max, q_max, kv_max, kv_max, h->ws.total,
+                                sizeof(int32_t) * (size_t)c.max_requests * c.max_pages_per_req,
+                                sizeof(int32_t) * (size_t)(c.max_requests + 1), sizeof(int32_t) * (size_t)c.max_requests};
+        cudaError_t e = cudaSuccess;
+        for (int i = 0; i < 8 && e == cudaSuccess; ++i) e = cudaMalloc(slots[i], sizes[i]);
+        if (e != cudaSuccess) {
+            for (int i = 0; i < 8; ++i) {
+                if (*slots[i]) cudaFree(*slots[i]);
+                *slots[i] = nullptr;
+            }
+            return fail_cuda(h, e, "staging alloc");
+        }
     }
     const size_t q_bytes = (size_t)T * c.num_q_heads * c.head_dim * 2;
     const size_t kv_bytes = (size_t)T * c.num_kv_heads * c.head_dim * 2;

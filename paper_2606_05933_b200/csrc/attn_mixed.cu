@@ -6,15 +6,15 @@
 // costs ~max(bytes/HBM, flops/tensor) instead of the sum.  6 warps per CTA:
 //   warp 0      scheduler + TMA producer.  Publishes each item to the other warps through a 4-slot smem
 //               ring, loads the Q tile (prefill) and streams 128-key K and V tiles — 8 pages x D/64 boxes of
-//               16 rows x 128 B, SWIZZLE_128B — into separate 2-slot K and V rings (K of tile t+2 can land
+//               16 rows x 128 B, SWIZZLE_128B — into separate 3-slot K and V rings (K of a later tile can land
 //               as soon as S(t) is done, V as soon as PV(t) is done).
 //   warp 1      tcgen05.mma issuer + TMEM owner (prefill items only):
 //                 S[b] (128x128 fp32, TMEM cols 128b..) = Q K^T,  double buffered so softmax(t) overlaps S(t+1)
-//                 O    (128xD  fp32, TMEM cols 256..)  += P[b] V  (P from swizzled smem, V MN-major)
+//                 O    (128xD  fp32, TMEM cols 256..)  += P[b] V  (P as bf16 pairs in TMEM, V MN-major in smem)
 //   warps 2..5  workers.
 //               prefill item: thread = query row (TMEM lane): tcgen05.ld S, causal/length mask by select,
 //                 online softmax (exp2, log2e folded into the scale, lazy rescale: O is only touched when a
-//                 row max grows by more than 2^8), P -> bf16 -> smem, epilogue stores rows < nrows only.
+//                 row max grows by more than 2^8), P -> bf16 -> TMEM, epilogue stores rows < nrows only.
 //               decode item: warp w owns keys [32w,32w+32) of each tile: mma.sync.m16n8k16 with the G query
 //                 heads of the KV head padded to 16 rows (bandwidth-bound, wasted rows are free), online
 //                 softmax in registers with quad shuffles, cross-warp log-sum-exp merge through smem, then
@@ -106,6 +106,7 @@ struct MixParams {
     int self_plan, R, num_sms, force_split_keys, force_decode_ctas;
     unsigned long long* trace;     // ss_debug_set_trace: per-CTA timeline, or null
     int trace_words;
+    const int32_t* err_flag;       // SS_FLAG_DEBUG_CHECKS: nonzero = the metadata check tripped, serve no item; else null
 };
 
 template <int D>
@@ -168,7 +169,11 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     PlanTables<uint16_t> ptb;
     ptb.ord = reinterpret_cast<uint16_t*>(smem + SM::kPlanOff + 64);
     ptb.off = ptb.ord + kPlanMaxR;
-    if (prm.self_plan) {
+    const bool tripped = prm.err_flag && *reinterpret_cast<const volatile int32_t*>(prm.err_flag) != 0;   // CTA-uniform
+    if (tripped) {
+        // debug checks found bad metadata: an empty plan - every role sees the end-of-list item and leaves
+        if (threadIdx.x == 0) { ph->tot_p = 0; ph->tot_d = 0; ph->n_decode_ctas = 0; ph->nP = 0; ph->nD = 0; }
+    } else if (prm.self_plan) {
         // a2: every CTA builds the same plan (scratch = the still unused K ring); items are decoded from queue tickets
         build_plan<kMixThreads, uint16_t>(prm.qsl, prm.ctx_lens, prm.R, Hq, Hkv, D, prm.num_sms, prm.force_split_keys,
                                           prm.force_decode_ctas, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph);
@@ -813,7 +818,8 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     p.hdr = (WorkHeader*)(ws + h->ws.header_off);
     p.items = (const ss_work_item*)(ws + h->ws.items_off);
     p.self_plan = main_self_plans(h, R, T) ? 1 : 0;
-    p.merge_counters = p.self_plan ? h->state + 4 : (int32_t*)(ws + h->ws.counters_off);
+    p.merge_counters = p.self_plan ? h->state + kStateCounters : (int32_t*)(ws + h->ws.counters_off);
+    p.err_flag = h->debug_checks ? h->state + kStateErr : nullptr;
     p.queue = p.self_plan ? h->state : &p.hdr->next_prefill;
     p.qsl = qsl;
     p.R = R;
@@ -833,22 +839,19 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     *n_launches = 1;
     const int grid = h->dbg[kDbgGrid] > 0 ? h->dbg[kDbgGrid] : h->num_sms;
     cudaError_t e;
-    if (c.head_dim == 128) {
-        auto kern = mixed_kernel<128>;
-        constexpr int smem = MixSmem<128>::kTotal;
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        e = launch_pdl(kern, dim3(grid), dim3(kMixThreads), smem, stream, tmap_q, h->tmap_k, h->tmap_v, p);
-        if (e != cudaSuccess) return e;
-    } else {
-        auto kern = mixed_kernel<64>;
-        constexpr int smem = MixSmem<64>::kTotal;
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        e = launch_pdl(kern, dim3(grid), dim3(kMixThreads), smem, stream, tmap_q, h->tmap_k, h->tmap_v, p);
-        if (e != cudaSuccess) return e;
-    }
+    if (c.head_dim == 128)
+        e = launch_pdl(mixed_kernel<128>, dim3(grid), dim3(kMixThreads), MixSmem<128>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+    else
+        e = launch_pdl(mixed_kernel<64>, dim3(grid), dim3(kMixThreads), MixSmem<64>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
+}
+
+// Opt in to the large dynamic shared-memory window once per process and head_dim (ss_create), not per call.
+cudaError_t init_main_attention(int head_dim) {
+    if (head_dim == 128)
+        return cudaFuncSetAttribute(mixed_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, MixSmem<128>::kTotal);
+    return cudaFuncSetAttribute(mixed_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, MixSmem<64>::kTotal);
 }
 
 }  // namespace ss

@@ -8,6 +8,7 @@
 #include <stdio.h>
 
 #include "slidingattn.h"
+#include "slidingattn_debug.h"
 
 namespace ss {
 
@@ -42,7 +43,13 @@ struct WorkHeader {
 struct WorkspaceLayout {
     size_t header_off, items_off, counters_off, partial_off, total;
     int32_t max_items, max_partials;
+    bool ok;                         // false: the config's worst case does not fit the int32 item / slot index space
 };
+
+constexpr int kStateErr = 4;         // Handle::state word offsets
+constexpr int kStateCounters = 8;
+// debug-check codes (ss_poll_device_error)
+enum { kChkQsl = 1, kChkCtxNegative = 2, kChkTooManyPages = 3, kChkPageId = 4 };
 
 struct Handle {
     ss_config cfg;
@@ -60,7 +67,10 @@ struct Handle {
     int last_launches;
     int force_simple;
     int dbg[8];                      // ss_debug_set_param knobs (0 = automatic)
-    int32_t* state;                  // device: [0..3] self-cleaning queue tickets, [4..) split arrival counters (max_requests*Hkv)
+    int32_t* state;                  // device: [0..3] self-cleaning queue tickets, [4..7] debug-check record (code, request,
+                                     // value, limit), [8..) split arrival counters (max_requests*Hkv)
+    size_t state_bytes;
+    int debug_checks;                // SS_FLAG_DEBUG_CHECKS: validate device metadata before every hot call
     unsigned long long* trace;       // ss_debug_set_trace buffer (device) or null
     int trace_words;
     int timing_on, timing_valid;
@@ -78,8 +88,9 @@ inline WorkspaceLayout workspace_layout(const ss_config& c, int num_sms) {
     const int64_t max_ctx = (int64_t)c.max_pages_per_req * kPage;
     const int64_t max_decode = (int64_t)c.num_kv_heads * c.max_requests * ((max_ctx + kMaxSplitKeys - 1) / kMaxSplitKeys + 1) +
                                (int64_t)num_sms * kDecodeWaves + 64;
-    w.max_items = (int32_t)(max_prefill + max_decode);
-    w.max_partials = (int32_t)max_decode;
+    w.ok = max_prefill + max_decode <= (int64_t)0x7fffffff / 4;     // item / partial-slot indices stay far inside int32
+    w.max_items = (int32_t)(w.ok ? max_prefill + max_decode : 0);
+    w.max_partials = (int32_t)(w.ok ? max_decode : 0);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = (off + bytes + 255) & ~(size_t)255; return o; };
     w.header_off = take(sizeof(WorkHeader));
@@ -117,6 +128,11 @@ cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_
                                     const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
                                     cudaStream_t stream, int prefill_only = 0);
 bool main_self_plans(const Handle* h, int R, int T);
+cudaError_t init_main_attention(int head_dim);           // one-time function attributes (ss_create)
+// SS_FLAG_DEBUG_CHECKS: device-side validation of (qsl, ctx_lens, block_table); records the first violation in
+// h->state[kStateErr..] - the hot kernels of this and later calls then skip every cache / output access
+cudaError_t launch_validate(const Handle* h, const int32_t* bt, const int32_t* qsl, const int32_t* ctx, int R, int T,
+                            cudaStream_t stream);
 // Main path (a3 + a4 + a5): consumes the work list in `workspace`; *n_launches receives the kernel count.
 cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
                                   const int32_t* ctx, int R, int T, float scale, void* out, float* lse,

@@ -11,9 +11,11 @@ __global__ void __launch_bounds__(128)
 kv_append_kernel(const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
                  uint4* __restrict__ k_cache, uint4* __restrict__ v_cache,
                  const int32_t* __restrict__ block_table, const int32_t* __restrict__ qsl,
-                 const int32_t* __restrict__ ctx_lens, int R, int max_pages, int Hkv, int vec_per_head) {
+                 const int32_t* __restrict__ ctx_lens, int R, int max_pages, int Hkv, int vec_per_head,
+                 const int32_t* __restrict__ err_flag) {
     ptx::pdl_launch_dependents();
     ptx::pdl_wait();
+    if (err_flag && *reinterpret_cast<const volatile int32_t*>(err_flag)) return;    // debug checks tripped: write nothing
     const int tok = blockIdx.x;
     const uint4* __restrict__ src = blockIdx.y ? v_new : k_new;
     uint4* __restrict__ dst = blockIdx.y ? v_cache : k_cache;
@@ -45,7 +47,7 @@ cudaError_t launch_kv_append(const Handle* h, const void* k_new, const void* v_n
     dim3 grid((unsigned)T, 2, 1);
     return launch_pdl(kv_append_kernel, grid, dim3(128), 0, stream, (const uint4*)k_new, (const uint4*)v_new,
                       (uint4*)h->k_cache, (uint4*)h->v_cache, bt, qsl, ctx, R, c.max_pages_per_req, c.num_kv_heads,
-                      c.head_dim / 8);
+                      c.head_dim / 8, (const int32_t*)(h->debug_checks ? h->state + kStateErr : nullptr));
 }
 
 }  // namespace ss

@@ -173,6 +173,25 @@ def config_c5(seed: int = 5, shuffle: bool = False) -> Batch:
                       shuffle_requests=shuffle)
 
 
+# Layer shapes (Hq, Hkv, D) of the models the paper serves ("Llama3-8B and Qwen2.5-7B", tensor parallel
+# degree 2 on its 2-GPU boxes), from the public model configs; SURVEY.md section 8(f) NEXT-3.  Qwen2.5-7B has 28 query
+# and 4 KV heads: G = 7, the first non-power-of-two group (TP2 slice: 14/2, also G = 7).
+MODEL_SHAPES = {
+    "llama3-8b": (32, 8, 128), "llama3-70b": (64, 8, 128), "qwen2.5-7b": (28, 4, 128),
+    "llama3-8b-tp2": (16, 4, 128), "qwen2.5-7b-tp2": (14, 2, 128),
+}
+
+
+def config_model_mixed(model: str, seed: int = 6, chunk: int = 512, chunk_ctx: int = 1024, n_decode: int = 64,
+                       shuffle: bool = False) -> Batch:
+    """C2's recipe (one chunk + decodes ctx U{512..4096}) on another model's layer shape."""
+    Hq, Hkv, D = MODEL_SHAPES[model]
+    rng = np.random.default_rng(seed)
+    dec = rng.integers(512, 4096, size=n_decode, endpoint=True)
+    reqs = [(chunk, chunk_ctx)] + [(1, int(u)) for u in dec]
+    return make_batch(f"MX-{model}", Hq, Hkv, D, reqs, seed, rng=rng, shuffle_requests=shuffle, with_append=True)
+
+
 SCENE_EDGES = {
     "PP-a": (32, 8, [(2048, 0)]),
     "PP-b": (32, 8, [(2048, 4096)]),
@@ -181,6 +200,7 @@ SCENE_EDGES = {
     "PP-e": (32, 8, [(8192, 0)]),
     "PP-f": (64, 8, [(1024, 0), (1024, 6000)]),
     "PP-g": (64, 8, [(4096, 4096)]),
+    "PP-q": (28, 4, [(2048, 4096)]),        # PP-b on the Qwen2.5-7B shape (G = 7)
 }
 
 

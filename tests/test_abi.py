@@ -16,30 +16,40 @@ def lib():
     return binding.load()
 
 
-def declared_symbols():
-    text = (ROOT / "include" / "slidingattn.h").read_text()
+def declared_symbols(header="slidingattn.h"):
+    text = (ROOT / "include" / header).read_text()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(ss_[a-z_]+)\s*\(", text)))
 
 
+# the product boundary is exactly this list (plus lifetime / status helpers)
+SECTION_8B = {"ss_create", "ss_destroy", "ss_workspace_bytes", "ss_kv_append", "ss_mixed_attention",
+              "ss_poll_device_error", "ss_status_string"}
+
+
 def test_header_declares_the_two_path_calls():
     syms = declared_symbols()
-    assert "ss_kv_append" in syms and "ss_mixed_attention" in syms and len(syms) >= 8
+    assert SECTION_8B <= set(syms)
+    assert not any(s.startswith("ss_debug") or "timing" in s or "worklist" in s for s in syms), \
+        "measurement / debug aids belong in slidingattn_debug.h"
 
 
 def test_library_exports_every_declared_symbol(lib):
     from paper_2606_05933_b200 import binding
-    for name in declared_symbols():
-        assert hasattr(lib, name), f"{name} declared in slidingattn.h but not exported"
+    for header in ("slidingattn.h", "slidingattn_debug.h"):
+        for name in declared_symbols(header):
+            assert hasattr(lib, name), f"{name} declared in {header} but not exported"
     assert sorted(binding.EXPORTS) == declared_symbols()
+    assert sorted(binding.DEBUG_EXPORTS) == declared_symbols("slidingattn_debug.h")
 
 
 def test_version_and_status_strings(lib):
-    assert lib.ss_version() == 100
+    assert lib.ss_version() == 200
     assert lib.ss_status_string(0) == b"SS_OK"
     assert lib.ss_status_string(-1) == b"SS_ERR_INVALID_ARG"
     assert lib.ss_status_string(-2) == b"SS_ERR_WORKSPACE_TOO_SMALL"
     assert lib.ss_status_string(-3) == b"SS_ERR_UNSUPPORTED_DEVICE"
+    assert lib.ss_status_string(-6) == b"SS_ERR_DEVICE_CHECK"
 
 
 def test_null_arguments_are_rejected_without_a_device(lib):
@@ -56,6 +66,25 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.ss_create(ctypes.byref(h), ctypes.byref(bad), 256, 512) == -1
     assert lib.ss_kv_append(None, None, None, None, None, None, 1, 1, None) == -1
     assert lib.ss_workspace_bytes(None) == 0
+    assert lib.ss_poll_device_error(None, None) == -1 and lib.ss_reset(None, None) == -1
+    bad = ss_config(32, 8, 128, 16, 64, 4, 64, 8, 2)         # unknown flag bit
+    assert lib.ss_create(ctypes.byref(h), ctypes.byref(bad), 256, 512) == -1
+    bad = ss_config(64, 8, 128, 16, 64, 2048, 2 ** 31 - 1, 2 ** 26)   # worst-case item count overflows int32
+    assert lib.ss_create(ctypes.byref(h), ctypes.byref(bad), 256, 512) == -1
+
+
+def test_binding_refuses_wrong_dtypes_and_shapes():
+    """torch's default int64 index tensors must not reach the raw-pointer ABI."""
+    import torch
+    from paper_2606_05933_b200 import binding
+    with pytest.raises(binding.SlidingAttnError, match="int32"):
+        binding._want(torch.zeros(4, dtype=torch.int64), "ctx_lens", torch.int32, cuda=False)
+    with pytest.raises(binding.SlidingAttnError, match="contiguous"):
+        binding._want(torch.zeros(4, 4, dtype=torch.int32)[:, ::2], "block_table", torch.int32, cuda=False)
+    with pytest.raises(binding.SlidingAttnError, match="shape"):
+        binding._want(torch.zeros(5, dtype=torch.int32), "query_start_loc", torch.int32, cuda=False, shape=(4,))
+    with pytest.raises(binding.SlidingAttnError, match="CUDA"):
+        binding._want(torch.zeros(4, dtype=torch.int32), "ctx_lens", torch.int32, cuda=True)
 
 
 def test_binding_refuses_cpu_tensors(lib):

@@ -92,7 +92,11 @@ def test_c1_tiny(simple):
 
 
 @pytest.mark.parametrize("seed", range(6))
-@pytest.mark.parametrize("shape", [(8, 2, 128), (4, 4, 64), (32, 8, 128), (16, 2, 128), (8, 8, 64)])
+@pytest.mark.parametrize("shape", [(8, 2, 128), (4, 4, 64), (32, 8, 128), (16, 2, 128), (8, 8, 64),
+                                   # head_dim 64 with a GQA group (staged Q copy, 16-row MMA padding, a5 merge at D = 64)
+                                   (8, 4, 64), (16, 4, 64), (16, 2, 64), (32, 2, 64),
+                                   # G = 7 (Qwen2.5-7B 28/4 and its TP2 slice 14/2), G = 4 TP2 slice of Llama-3-8B, odd G = 3, 5
+                                   (28, 4, 128), (14, 2, 128), (16, 4, 128), (6, 2, 128), (10, 2, 64)])
 def test_random_ragged_batches(seed, shape):
     Hq, Hkv, D = shape
     b = wl.random_batch(1000 + 17 * seed + Hq, Hq=Hq, Hkv=Hkv, D=D, n_prefill=3, n_decode=6, max_c=300, max_u=700)
@@ -248,7 +252,7 @@ def test_chunking_invariance_on_gpu(chunks):
     check(full, torch.cat(outs), ref)
 
 
-def test_bitwise_reproducible_and_order_invariant_within_tolerance():
+def test_bitwise_reproducible_run_to_run():
     b = wl.random_batch(4242, Hq=32, Hkv=8, D=128, n_prefill=2, n_decode=8, max_c=260, max_u=3000, with_append=False)
     t = wl.make_tensors(b, DEV)
     o1, _, h = gpu_run(b, t)
@@ -308,8 +312,17 @@ def test_worklist_partitions_the_batch():
     assert len(spans) == sum(1 for c, _ in b.reqs if c == 1) * 8
     assert len(slots) <= n_part          # partial slots share the decode items' index space
     assert (covered == 1).all()
-    # heavy-first inside each kind
-    assert (np.diff(pre["kv_end"][::64].astype(np.int64)) <= 128).all() or True
+    # heavy-first inside each kind: prefill requests by KV length (u + c), and inside a request the last (heaviest)
+    # row tile first; the 64 heads of one (request, row tile) are consecutive
+    first_head = pre[::64]
+    assert (pre["head"].reshape(-1, 64) == np.arange(64)).all()
+    big = [r for r in np.unique(first_head["req"])]
+    req_order = list(dict.fromkeys(int(r) for r in first_head["req"]))
+    kv_len = [b.reqs[r][0] + b.reqs[r][1] for r in req_order]
+    assert kv_len == sorted(kv_len, reverse=True)
+    for r in req_order:
+        ends = first_head["kv_end"][first_head["req"] == r].astype(np.int64)
+        assert (np.diff(ends) < 0).all()
     lens = (dec["kv_end"] - dec["kv_begin"]).astype(np.int64)
     first_of_req = lens[::8]
     assert first_of_req[0] == lens.max()
@@ -348,24 +361,29 @@ def sampled_parity(b, n_rows, seed, poison=False):
     check(b, out, ref, lse, lse_ref, rows=rows)
 
 
-def test_c4_decode_heavy_full_pool_sampled_rows():
-    sampled_parity(wl.config_c4(), n_rows=48, seed=4)
-
-
-def test_c5_70b_mixed_with_append_sampled_rows():
-    b = wl.config_c5()
+def all_rows_parity_compacted(b):
+    """Every output row against the oracle, for batches whose pool does not fit the host: the oracle runs on the
+    pages the block table names (compact_pool; legal by the pinned page-permutation invariance)."""
     t = wl.make_tensors(b, DEV)
-    k0, v0 = wl.to_u16(t.k_cache), wl.to_u16(t.v_cache)
     out, lse, h = gpu_run(b, t)
-    oracle.kv_append(k0, v0, wl.to_u16(t.k_new), wl.to_u16(t.v_new), b.block_table, b.query_start_loc, b.ctx_lens)
-    assert np.array_equal(wl.to_u16(t.k_cache), k0) and np.array_equal(wl.to_u16(t.v_cache), v0)
-    rng = np.random.default_rng(5)
-    rows = sorted({0, 1, 127, 128, 1023, 1024, 1025, 2047} | set(int(x) for x in rng.choice(b.T, size=40, replace=False))
-                  | set(range(2048, 2048 + 12)))
-    rows = np.array(rows, dtype=np.int32)
-    ref, lse_ref, _ = oracle.mixed_attention(wl.to_u16(t.q), k0, v0, b.block_table, b.query_start_loc, b.ctx_lens, b.scale, rows=rows)
-    assert not torch.isnan(out.float()).any()
-    check(b, out, ref, lse, lse_ref, rows=rows)
+    bt2, (k, v) = wl.compact_pool(b, t.k_cache, t.v_cache)
+    ref, lse_ref, _ = oracle.mixed_attention(wl.to_u16(t.q), k, v, bt2, b.query_start_loc, b.ctx_lens, b.scale)
+    check(b, out, ref, lse, lse_ref)
+
+
+def test_c4_decode_heavy_full_pool_all_rows():
+    """BASELINE.json configs[3]: 256 decodes over the 2 x 20 GB pool, every row checked (38 GFLOP of fp64)."""
+    all_rows_parity_compacted(wl.config_c4())
+
+
+def test_c5_70b_mixed_with_append_all_rows():
+    """BASELINE.json configs[4] in bench.py's launch configuration: kv_append bit-exact over the whole pool, then all
+    2240 rows (incl. the 30 136-key decode that takes 8 KV splits) against the oracle."""
+    full_parity(wl.config_c5(), poison=False)
+
+
+def test_c5_shuffled_request_order_poisoned():
+    full_parity(wl.config_c5(shuffle=True), poison=True)
 
 
 @pytest.mark.parametrize("C,n,N_d", [(256, 3, 32), (2048, 1, 32), (1024, 4, 128), (0, 1, 128)])
@@ -375,6 +393,145 @@ def test_c3_grid_points(C, n, N_d):
 
 def test_scene_edge_pure_prefill_sampled():
     sampled_parity(wl.config_scene_edge("PP-d"), n_rows=64, seed=9)
+
+
+@pytest.mark.parametrize("name", ["PP-b", "PP-f", "PP-q"])
+def test_scene_edges_the_tensor_roofline_is_quoted_on_all_rows(name):
+    """PP-b (2048 on 4096, 8B shape), PP-f (70B shape, G = 8 prefill), PP-q (Qwen shape, G = 7): every row."""
+    full_parity(wl.config_scene_edge(name), poison=False)
+
+
+def tile_edge_rows(b):
+    """Rows 0, 127, 128, last, and the first/last row of every 128-row tile of every prefill chunk."""
+    rows = set()
+    for r, (c, u) in enumerate(b.reqs):
+        s0 = int(b.query_start_loc[r])
+        if c > 1:
+            rows.update(s0 + j for j in range(0, c, 128))
+            rows.update(s0 + min(j + 127, c - 1) for j in range(0, c, 128))
+        elif c == 1:
+            rows.add(s0)
+    return rows
+
+
+@pytest.mark.parametrize("name", ["PP-e", "PP-g"])
+def test_scene_edges_many_row_tiles_sampled(name):
+    """PP-e: 8192 rows = 64 row tiles; PP-g: 70B shape (4096, 4096).  Tile-edge rows forced + a random sample."""
+    b = wl.config_scene_edge(name)
+    t = wl.make_tensors(b, DEV)
+    out, lse, h = gpu_run(b, t)
+    rng = np.random.default_rng(11)
+    rows = tile_edge_rows(b) | set(int(x) for x in rng.choice(b.T, size=96, replace=False))
+    rows = np.array(sorted(rows), dtype=np.int32)
+    ref, lse_ref, _ = oracle.mixed_attention(wl.to_u16(t.q), wl.to_u16(t.k_cache), wl.to_u16(t.v_cache), b.block_table,
+                                             b.query_start_loc, b.ctx_lens, b.scale, rows=rows)
+    assert not torch.isnan(out.float()).any()
+    check(b, out, ref, lse, lse_ref, rows=rows)
+
+
+@pytest.mark.parametrize("model", ["qwen2.5-7b", "qwen2.5-7b-tp2", "llama3-8b-tp2"])
+def test_next3_model_shapes_mixed(model):
+    """the Qwen2.5-7B layer (28/4/128, G = 7) and the TP2 per-GPU slices the paper ran
+    (PAPER.md:382), C2's recipe, with append."""
+    full_parity(wl.config_model_mixed(model), poison=True)
+    full_parity(wl.config_model_mixed(model, shuffle=True), poison=False)
+
+
+def test_batch_composition_invariance_on_gpu():
+    """requests share a batch but are independent.  A prefill chunk and a decode of C2 run (i) inside C2
+    and (ii) alone; both times the rows match the oracle's rows for that request (which the oracle pins bitwise
+    against composition), and the two GPU results agree to within twice the tolerance."""
+    b = wl.config_c2()
+    t = wl.make_tensors(b, DEV)
+    out_full, _, _ = gpu_run(b, t, lse=False)
+    ref_full, _, _ = oracle.mixed_attention(wl.to_u16(t.q), wl.to_u16(t.k_cache), wl.to_u16(t.v_cache), b.block_table,
+                                            b.query_start_loc, b.ctx_lens, b.scale)
+    longest = int(np.argmax([u if c == 1 else -1 for c, u in b.reqs]))
+    for r in (0, 1, longest, b.R - 1):
+        c, u = b.reqs[r]
+        s0 = int(b.query_start_loc[r])
+        solo = wl.Batch(f"solo{r}", b.num_q_heads, b.num_kv_heads, b.head_dim, [(c, u)], b.num_pages,
+                        np.ascontiguousarray(b.block_table[r:r + 1]), np.array([0, c], dtype=np.int32),
+                        np.array([u], dtype=np.int32), b.seed)
+        ts = wl.Tensors(t.q[s0:s0 + c].contiguous(), None, None, t.k_cache, t.v_cache)
+        out_solo, _, _ = gpu_run(solo, ts, lse=False)
+        ref = ref_full[s0:s0 + c]
+        for got in (out_solo, out_full[s0:s0 + c]):
+            err = np.abs(got.to(torch.float64).cpu().numpy() - ref)
+            assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS
+            assert np.linalg.norm(got.to(torch.float64).cpu().numpy() - ref) / np.linalg.norm(ref) <= REL_L2
+        assert (out_solo.float() - out_full[s0:s0 + c].float()).abs().max().item() <= 2 * MAX_ABS
+
+
+def test_scale_must_be_finite_and_positive():
+    """slidingattn.h: scale <= 0 or non-finite is SS_ERR_INVALID_ARG (the kernels take the running max of raw scores).
+    A tiny positive scale is the GPU twin of the oracle's scale = 0 closed form: every row -> prefix mean of V."""
+    b = wl.random_batch(31, Hq=8, Hkv=2, D=128, n_prefill=2, n_decode=4, max_c=150, max_u=400, with_append=False)
+    t = wl.make_tensors(b, DEV, poison_unused=True)
+    h = binding.handle_for(b, t)
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    for bad in (0.0, -0.125, float("nan"), float("inf"), -float("inf")):
+        with pytest.raises(binding.SlidingAttnError) as ei:
+            binding.mixed_attention(h, t.q, bt, qsl, ctx, bad)
+        assert ei.value.status == binding.SS_ERR_INVALID_ARG
+    out = binding.mixed_attention(h, t.q, bt, qsl, ctx, 1e-30)
+    torch.cuda.synchronize()
+    ref, _, _ = oracle.mixed_attention(wl.to_u16(t.q), wl.to_u16(t.k_cache), wl.to_u16(t.v_cache), b.block_table,
+                                       b.query_start_loc, b.ctx_lens, 0.0)
+    check(b, out, ref)
+
+
+# ------------------------------------------------------------------------------------------------
+# boundary: debug checks (SURVEY.md section 8(b)) and handle reset
+# ------------------------------------------------------------------------------------------------
+def _poisoned_metadata_cases(b):
+    bt, qsl, ctx = b.block_table.copy(), b.query_start_loc.copy(), b.ctx_lens.copy()
+    r = next(i for i, (c, u) in enumerate(b.reqs) if c == 1 and u > 40)
+    bad_page = bt.copy(); bad_page[r, 1] = b.num_pages + 7
+    neg_page = bt.copy(); neg_page[r, 0] = -3
+    bad_qsl = qsl.copy(); bad_qsl[2], bad_qsl[3] = bad_qsl[3] + 1, bad_qsl[2]
+    bad_end = qsl.copy(); bad_end[-1] += 1
+    too_long = ctx.copy(); too_long[r] = b.max_pages_per_req * 16 + 5
+    neg_ctx = ctx.copy(); neg_ctx[r] = -1
+    return {"page id >= num_pages": (bad_page, qsl, ctx, 4), "negative page id": (neg_page, qsl, ctx, 4),
+            "qsl not monotone": (bt, bad_qsl, ctx, 1), "qsl[R] != T": (bt, bad_end, ctx, 1),
+            "too many pages": (bt, qsl, too_long, 3), "negative ctx": (bt, qsl, neg_ctx, 2)}
+
+
+def test_debug_checks_flag_bad_metadata_and_skip_the_access():
+    b = wl.random_batch(77, Hq=8, Hkv=2, D=128, n_prefill=2, n_decode=6, max_c=200, max_u=500)
+    t = wl.make_tensors(b, DEV)
+    h = binding.handle_for(b, t, debug_checks=True)
+    k_before, v_before = t.k_cache.clone(), t.v_cache.clone()
+    for what, (bt_h, qsl_h, ctx_h, code) in _poisoned_metadata_cases(b).items():
+        out = torch.full_like(t.q, 7.0)
+        binding.kv_append(h, t.k_new, t.v_new, dev(bt_h), dev(qsl_h), dev(ctx_h))
+        binding.mixed_attention(h, t.q, dev(bt_h), dev(qsl_h), dev(ctx_h), b.scale, out=out)
+        with pytest.raises(binding.SlidingAttnError, match=f"device check {code}") as ei:
+            h.poll_device_error()
+        assert ei.value.status == binding.SS_ERR_DEVICE_CHECK, what
+        assert torch.equal(t.k_cache, k_before) and torch.equal(t.v_cache, v_before), f"{what}: cache written"
+        assert bool((out == 7.0).all()), f"{what}: out written"
+        h.poll_device_error()                         # cleared: a second poll is clean
+    # the same handle then serves a good batch, and matches the oracle
+    k0, v0 = wl.to_u16(t.k_cache), wl.to_u16(t.v_cache)
+    out, lse, _ = gpu_run(b, t, handle=h)
+    h.poll_device_error()
+    oracle.kv_append(k0, v0, wl.to_u16(t.k_new), wl.to_u16(t.v_new), b.block_table, b.query_start_loc, b.ctx_lens)
+    assert np.array_equal(wl.to_u16(t.k_cache), k0) and np.array_equal(wl.to_u16(t.v_cache), v0)
+    ref, lse_ref, _ = oracle.mixed_attention(wl.to_u16(t.q), k0, v0, b.block_table, b.query_start_loc, b.ctx_lens, b.scale)
+    check(b, out, ref, lse, lse_ref)
+    assert h.last_launch_count() == 2                 # validate + main launch
+
+
+def test_poll_is_clean_without_debug_checks_and_reset_rearms_the_handle():
+    b = wl.random_batch(78, Hq=8, Hkv=2, D=128, n_prefill=1, n_decode=5, max_c=100, max_u=3000, with_append=False)
+    t = wl.make_tensors(b, DEV)
+    out1, _, h = gpu_run(b, t, lse=False)
+    h.poll_device_error()
+    h.reset()
+    out2, _, _ = gpu_run(b, t, lse=False, handle=h)
+    assert torch.equal(out1, out2)
 
 
 def test_iteration_host_matches_device_path():

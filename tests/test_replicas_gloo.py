@@ -53,3 +53,20 @@ def test_single_rank_needs_no_process_group():
     import bench
     assert bench.max_over_ranks(3.5, 1) == 3.5
     assert bench.replica_metric(30.0, 10, 1) == (3.0, 3000.0)
+
+
+def test_bench_gpus_n_spawns_its_own_ranks():
+    """`python bench.py --gpus 2` without torchrun re-executes itself under torch.distributed.run (it used
+    to time one replica and print n_gpus 1).  --dry-run keeps the kernels out so this runs on CPU over gloo."""
+    import json
+    import subprocess
+    root = Path(__file__).resolve().parent.parent
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, str(root / "bench.py"), "--gpus", "2", "--dry-run", "--steps", "5"],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=root)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [json.loads(l) for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, res.stdout                      # rank 0 alone prints
+    line = lines[0]
+    assert line["n_gpus"] == 2 and line["steps"] == 5
+    assert line["ms_per_step"] == 20.0 and line["value"] == 10000.0     # slowest rank: 20 ms per step, 2 replicas
