@@ -294,10 +294,11 @@ class Bench:
         del self.t, self.out, self.h
         torch.cuda.empty_cache()
 
-    def time_steps(self, steps: int, warmup: int, flush, barrier=lambda: None):
+    def time_steps(self, steps: int, warmup: int, flush, barrier=None):
         """(per-step ms array, launches per step, wall seconds): CUDA events per step on the launching stream, L2
         flushed between steps outside the event window."""
         import torch
+        barrier = barrier or torch.cuda.synchronize
         stream = torch.cuda.current_stream()
         launches = 0
         for _ in range(max(warmup, 3)):
