@@ -13,7 +13,7 @@ extern "C" {
 
 /* One entry of the device work list (a2); exposed so tests can check the builder.
  * kind 1 = prefill tile: query rows [row0, row0+nrows) of request req (c_r > 1, Eq. 2),
- *          query head `head`, keys [0, kv_end);
+ *          query heads head .. head+nheads-1 (1 or 2 heads of one KV head), keys [0, kv_end);
  * kind 2 = decode split: the single row of request req (c_r == 1), KV head `head`, keys
  *          [kv_begin, kv_end); partial results go to slot `partial` unless nsplit == 1. */
 typedef struct ss_work_item {
@@ -28,7 +28,7 @@ typedef struct ss_work_item {
     int32_t nsplit;
     int32_t partial;    /* decode: first partial slot of this (req, kv head), slot = partial + split */
     int32_t q_pos0;     /* prefill: chunk-relative index j of the first row (row j sees keys 0..u+j) */
-    int32_t reserved;
+    int32_t nheads;     /* prefill: 1 or 2 query heads served by the item; decode: the G heads of the KV head */
 } ss_work_item;
 
 /*

@@ -38,7 +38,7 @@ class ss_config(ctypes.Structure):
 class ss_work_item(ctypes.Structure):
     _fields_ = [(n, ctypes.c_int32) for n in
                 ("kind", "req", "head", "row0", "nrows", "kv_begin", "kv_end", "split", "nsplit",
-                 "partial", "q_pos0", "reserved")]
+                 "partial", "q_pos0", "nheads")]
 
 
 WORK_ITEM_DTYPE = np.dtype([(n, np.int32) for n, _ in ss_work_item._fields_])

@@ -3,23 +3,30 @@
 //
 // Persistent CTAs (one per SM) pull items from the device work list through a dynamic queue (atomic
 // counter), so tensor-bound prefill tiles and HBM-bound decode splits overlap across SMs and the batch
-// costs ~max(bytes/HBM, flops/tensor) instead of the sum.  6 warps per CTA:
-//   warp 0      scheduler + TMA producer.  Publishes each item to the other warps through a 4-slot smem
-//               ring, loads the Q tile (prefill) and streams 128-key K and V tiles — 8 pages x D/64 boxes of
-//               16 rows x 128 B, SWIZZLE_128B — into separate 3-slot K and V rings (K of a later tile can land
-//               as soon as S(t) is done, V as soon as PV(t) is done).
-//   warp 1      tcgen05.mma issuer + TMEM owner (prefill items only):
-//                 S[b] (128x128 fp32, TMEM cols 128b..) = Q K^T,  double buffered so softmax(t) overlaps S(t+1)
-//                 O    (128xD  fp32, TMEM cols 256..)  += P[b] V  (P as bf16 pairs in TMEM, V MN-major in smem)
-//   warps 2..5  workers.
-//               prefill item: thread = query row (TMEM lane): tcgen05.ld S, causal/length mask by select,
-//                 online softmax (exp2, log2e folded into the scale, lazy rescale: O is only touched when a
-//                 row max grows by more than 2^8), P -> bf16 -> TMEM, epilogue stores rows < nrows only.
-//               decode item: warp w owns keys [32w,32w+32) of each tile: mma.sync.m16n8k16 with the G query
-//                 heads of the KV head padded to 16 rows (bandwidth-bound, wasted rows are free), online
-//                 softmax in registers with quad shuffles, cross-warp log-sum-exp merge through smem, then
-//                 either the final bf16 row or an fp32 partial; the CTA that writes the last partial of a
-//                 (request, kv head) merges all of them in fixed split order (bitwise reproducible).
+// costs ~max(bytes/HBM, flops/tensor) instead of the sum.  12 warps per CTA in 3 warpgroups; the register
+// file is re-partitioned with setmaxnreg (WG0 80 registers per thread, WG1 / WG2 216):
+//   WG0 warp 0  scheduler + TMA producer (one elected thread).  Publishes each item to the other warps through a
+//               4-slot smem ring, loads the Q tiles (prefill: the item's 1 or 2 query heads, 128 rows each) and
+//               streams 64-key K and V tiles — 4 pages x D/64 boxes of 16 rows x 128 B, SWIZZLE_128B — into
+//               separate 5-slot K and V rings (a K slot is free as soon as its S MMAs are done, a V slot as soon
+//               as its PV MMAs are done).
+//   WG0 warp 1  tcgen05.mma issuer + TMEM owner (prefill items only), one elected thread.  Per query head X (a
+//               "chain") TMEM holds S_X[0], S_X[1] (128 rows x 64 keys fp32, 64 columns each) and O_X (128 x D
+//               fp32): 2 x 256 = all 512 columns.  P (bf16 pairs) is written IN PLACE over its S buffer, so per
+//               chain the order is  S(k) -> softmax -> P(k) -> PV(k) -> S(k+2)  with S(k+1) already done: each
+//               chain's softmax never waits for the tensor pipe, and the two chains interleave on it
+//               (PV_A(k) S_A(k+2) PV_B(k) S_B(k+2) ...) while sharing every staged K/V tile.
+//   WG1, WG2    workers (4 warps each; warp % 4 = TMEM lane quarter).
+//               prefill item: WG1 = chain A (head), WG2 = chain B (head + 1); thread = query row (TMEM lane):
+//                 tcgen05.ld S, causal/length mask by select (only in the warp-uniform diagonal variant), online
+//                 softmax (exp2, log2e folded into the scale, packed f32x2 arithmetic, lazy rescale: O is only touched
+//                 when a row max grows by more than 2^8), P -> bf16 -> TMEM, epilogue stores rows < nrows only.
+//               decode item: WG1 warp w owns 32 keys of a pair of 64-key slots: mma.sync.m16n8k16 with the G query
+//                 heads of the KV head padded to 16 rows (bandwidth-bound, wasted rows are free), online softmax
+//                 in registers with quad shuffles, cross-warp log-sum-exp merge through smem, then either the
+//                 final bf16 row or an fp32 partial.  WG2 warp 0 runs a5 meanwhile: it publishes each split
+//                 (acq_rel ticket) and, when it draws the last ticket of a (request, kv head), merges all splits
+//                 in fixed order (bitwise reproducible).
 // Rooflines: decode items HBM (2*D*2 bytes per cached token per kv head), prefill items bf16 tensor
 // (4*D flop per visible (row,key) pair per head).  V rows at/after kv_end are zeroed in smem before any
 // PV product (unused slots may hold NaN; 0*NaN = NaN); masked scores are replaced, never multiplied.
@@ -31,9 +38,11 @@ namespace ss {
 
 using namespace ptx;
 
-constexpr int kMixThreads = 192;
-constexpr int kNumSt = 3;            // K ring slots = V ring slots
+constexpr int kMixThreads = 384;
+constexpr int kSlotKeys = 64;        // keys per K / V ring slot = keys per S buffer
+constexpr int kNumSt = 5;            // K ring slots = V ring slots
 constexpr int kSchedSlots = 4;
+constexpr int kRegsWg0 = 80, kRegsWorker = 216;      // 128*80 + 256*216 = 65536
 constexpr float kMLog2e = 1.4426950408889634f;
 constexpr float kMLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.f;   // log2 units: P <= 2^8, safe in bf16 / fp32
@@ -41,38 +50,42 @@ constexpr float kRescaleThreshold = 8.f;   // log2 units: P <= 2^8, safe in bf16
 template <int D>
 struct MixSmem {
     static constexpr int kHalves = D / 64;
-    static constexpr int kTile = kHalves * kTileKeys * 128;      // one K (or V, or Q) tile
+    static constexpr int kSlot = kHalves * kSlotKeys * 128;      // one K (or V) ring slot
+    static constexpr int kQTile = kHalves * kTileRows * 128;     // one Q tile (one query head, 128 rows)
     static constexpr int kKOff = 0;
-    static constexpr int kVOff = kKOff + kNumSt * kTile;
-    static constexpr int kQOff = kVOff + kNumSt * kTile;         // Q tile (prefill) / decode: cross-warp merge buffer + staged Q rows
+    static constexpr int kVOff = kKOff + kNumSt * kSlot;
+    static constexpr int kQOff = kVOff + kNumSt * kSlot;         // 2 Q tiles (prefill) / decode: cross-warp merge buffer + staged Q rows
+    static constexpr int kQBytes = 2 * kQTile;
     static constexpr int kMergeBytes = 4 * kMaxGroup * (D + 2) * 4;
     // decode with G <= 8: merge buffer of 8 rows per warp, then kSchedSlots staged Q blocks (G rows x D bf16, one per
     // scheduler slot, bulk-copied by the producer so the workers never wait on a cold global Q load)
     static constexpr int kMerge8Bytes = 4 * 8 * (D + 2) * 4;
     static constexpr int kQStageOff = kQOff + (kMerge8Bytes + 127) / 128 * 128;
     static constexpr int kQStageBytes = 8 * D * 2;
-    static constexpr int kQBytes = ((kTile > kMergeBytes ? kTile : kMergeBytes) + 1023) / 1024 * 1024;
+    static_assert(kMergeBytes <= kQBytes, "decode merge buffer must fit the Q region");
     static_assert(kQStageOff + kSchedSlots * kQStageBytes <= kQOff + kQBytes, "staged Q blocks must fit beside the merge buffer");
     static constexpr int kBarOff = kQOff + kQBytes;
-    static constexpr int kSchedOff = kBarOff + 320;              // kSchedSlots x 48 B
+    static constexpr int kSchedOff = kBarOff + 512;              // kSchedSlots x 48 B
     static constexpr int kTmemSlotOff = kSchedOff + kSchedSlots * 48;
     // in-kernel plan (plan.cuh): header + rank tables for up to kPlanMaxR requests, alive for the whole kernel
-    static constexpr int kPlanOff = kBarOff + 640;
+    static constexpr int kPlanOff = kTmemSlotOff + 32;
     static constexpr int kPlanBytes = 64 + 4 * kPlanMaxR;
     static constexpr int kTotal = kPlanOff + kPlanBytes;       // no alignment slack: the dynamic window is declared 1024-aligned
-    // TMEM columns: S0 [0,128) S1 [128,256) O [256,256+D) P0 [384,448) P1 [448,512) (P = bf16 pairs)
+    // TMEM columns per chain X (base 256 X): S[0] [0,64) S[1] [64,128) O [128,128+D); P[b] = first 32 columns of S[b]
     static constexpr int kTmemCols = 512;
-    static constexpr int kTmemO = 256, kTmemP = 384;
+    static constexpr int kTmemChain = 256, kTmemO = 128;
     static_assert(kTotal <= 232448, "shared memory budget");
 };
 
 // barrier indices (8 bytes each, from kBarOff)
 enum : int {
-    B_KFULL = 0, B_VFULL = 3, B_KEMPTY_P = 6, B_KEMPTY_D = 9, B_VEMPTY_P = 12, B_VEMPTY_D = 15,
-    B_SFULL = 18, B_PFULL = 20, B_QFULL = 22, B_QEMPTY = 23, B_OFULL = 24, B_OFREE = 25, B_PVDONE = 26,
-    B_SCHED_FULL = 27, B_SCHED_EMPTY = 31, B_PARTIAL = 35, B_COUNT = 39
+    B_KFULL = 0, B_VFULL = 5, B_KEMPTY_P = 10, B_KEMPTY_D = 15, B_VEMPTY_P = 20, B_VEMPTY_D = 25,
+    B_SFULL = 30, B_PFULL = 34,                       // [chain * 2 + buffer]
+    B_QFULL = 38, B_QEMPTY = 39, B_OFULL = 40, B_OFREE = 42, B_PVDONE = 44,     // [chain]
+    B_SCHED_FULL = 46, B_SCHED_EMPTY = 50, B_PARTIAL = 54, B_COUNT = 58
 };
-static_assert(B_COUNT * 8 <= 320, "barrier region");
+static_assert(B_COUNT * 8 <= 512, "barrier region");
+static_assert(kNumSt == 5, "barrier indices assume 5 ring slots");
 
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
     uint64_t d = 0;
@@ -109,6 +122,39 @@ struct MixParams {
     const int32_t* err_flag;       // SS_FLAG_DEBUG_CHECKS: nonzero = the metadata check tripped, serve no item; else null
 };
 
+// One 64-key half tile of one query row: S (64 fp32 scores in sr) -> P (bf16 pairs in pk), online-softmax state (m, l).
+// MASKED: keys at and after nvis are invisible (causal diagonal / end of the KV range); replaced by select.
+// Returns alpha (the factor the accumulated O row must be scaled by; 1 unless the reference max moved).
+template <bool MASKED>
+__device__ __forceinline__ float softmax_half(uint32_t (&sr)[2][32], int nvis, float sl2, float& m, float& l, uint32_t (&pk)[32]) {
+    float bm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int i = 0; i < 32; ++i) {
+            if (MASKED && c * 32 + i >= nvis) sr[c][i] = 0xff800000u;   // -inf by select, never by arithmetic
+            bm[i & 3] = fmaxf(bm[i & 3], __uint_as_float(sr[c][i]));
+        }
+    const float cand = fmaxf(fmaxf(bm[0], bm[1]), fmaxf(bm[2], bm[3])) * sl2;
+    // lazy rescale: only move the reference max when it grows by more than 2^8
+    float m_new = m, alpha = 1.f;
+    if (cand > m + kRescaleThreshold) { m_new = cand; alpha = exp2f(m - m_new); }   // first tile: m = -inf -> alpha = 0
+    const float2 sl2v = make_float2(sl2, sl2), nm = make_float2(-m_new, -m_new);
+    float2 ps[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+    // P = exp2(s*sl2 - m_new) -> bf16 pairs (A operand of the PV MMA), 32 packed columns per row
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+        const float2 x = __ffma2_rn(make_float2(__uint_as_float(sr[i >> 4][(2 * i) & 31]), __uint_as_float(sr[i >> 4][((2 * i) & 31) + 1])), sl2v, nm);
+        const float2 p = make_float2(exp2f(x.x), exp2f(x.y));
+        ps[i & 3] = __fadd2_rn(ps[i & 3], p);
+        pk[i] = pack_bf16(p.x, p.y);
+    }
+    const float2 s01 = __fadd2_rn(__fadd2_rn(ps[0], ps[1]), __fadd2_rn(ps[2], ps[3]));
+    l = l * alpha + (s01.x + s01.y);
+    m = m_new;
+    return alpha;
+}
+
 template <int D>
 __global__ void __launch_bounds__(kMixThreads, 1)
 mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
@@ -134,23 +180,25 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             mbar_init(BAR(B_KFULL + s), 1);
             mbar_init(BAR(B_VFULL + s), 1);
             mbar_init(BAR(B_KEMPTY_P + s), 1);
-            mbar_init(BAR(B_KEMPTY_D + s), 4);
+            mbar_init(BAR(B_KEMPTY_D + s), 2);
             mbar_init(BAR(B_VEMPTY_P + s), 1);
-            mbar_init(BAR(B_VEMPTY_D + s), 4);
+            mbar_init(BAR(B_VEMPTY_D + s), 2);
         }
-        for (int b = 0; b < 2; ++b) {
+        for (int b = 0; b < 4; ++b) {
             mbar_init(BAR(B_SFULL + b), 1);
             mbar_init(BAR(B_PFULL + b), 128);
         }
         mbar_init(BAR(B_QFULL), 1);
         mbar_init(BAR(B_QEMPTY), 1);
-        mbar_init(BAR(B_OFULL), 1);
-        mbar_init(BAR(B_OFREE), 128);
-        mbar_init(BAR(B_PVDONE), 1);
+        for (int x = 0; x < 2; ++x) {
+            mbar_init(BAR(B_OFULL + x), 1);
+            mbar_init(BAR(B_OFREE + x), 128);
+            mbar_init(BAR(B_PVDONE + x), 1);
+        }
         for (int s = 0; s < kSchedSlots; ++s) {
             mbar_init(BAR(B_PARTIAL + s), 128);
             mbar_init(BAR(B_SCHED_FULL + s), 1);
-            mbar_init(BAR(B_SCHED_EMPTY + s), 5);
+            mbar_init(BAR(B_SCHED_EMPTY + s), 9);                // MMA warp + 8 worker warps
         }
         fence_barrier_init();
         prefetch_tmap(&tmap_q);
@@ -186,10 +234,13 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     __syncthreads();
     if (trace && threadIdx.x == 0) trace[1] = globaltimer_ns();
     const uint32_t tmem_base = *tmem_slot;
-    const uint32_t tmem_o = tmem_base + SM::kTmemO;
-    const uint32_t tmem_p = tmem_base + SM::kTmemP;
 
-    if (warp == 0) {
+    // Re-partition the register file: the producer / issuer warpgroup gives up what the 8 worker warps need.  The two
+    // setmaxnreg sit INSIDE the role branches (which only re-join at the teardown): ptxas allocates each region against
+    // the count of the setmaxnreg that dominates it, and code reachable from both would get the smaller one.
+    if (warp < 4) {
+      setmaxnreg_dec<kRegsWg0>();
+      if (warp == 0) {
         // =============================== scheduler + TMA producer ===============================
         // One elected thread runs the whole loop (waits included) so every TMA operand is uniform.
         if (elect_one()) {
@@ -222,16 +273,16 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     wu.v[0] = wu.v[1] = wu.v[2] = make_uint4(0u, 0u, 0u, 0u);
                 }
             };
-            auto first_pages = [&](const ss_work_item& it, int (&pgs)[8]) {
+            auto first_pages = [&](const ss_work_item& it, int (&pgs)[4]) {
                 const int32_t* b = prm.block_table + (int64_t)it.req * prm.max_pages;
 #pragma unroll
-                for (int p = 0; p < 8; ++p)
+                for (int p = 0; p < 4; ++p)
                     pgs[p] = (it.kind != 0 && it.kv_begin + p * kPage < it.kv_end) ? __ldg(b + (it.kv_begin >> 4) + p) : 0;
             };
             // the NEXT item (queue ticket, record, first page ids) is fetched while the current item's tiles are being
             // issued, so the atomic -> record -> block-table latency chain never sits between two items' TMA streams
             WU nxt;
-            int nxt_pg[8];
+            int nxt_pg[4];
             fetch(nxt);
             first_pages(nxt.it, nxt_pg);
             for (;;) {
@@ -242,7 +293,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 dst[0] = wu.v[0]; dst[1] = wu.v[1]; dst[2] = wu.v[2];
                 const ss_work_item& w = wu.it;
                 if (w.kind == 2 && q_staged) {
-                    // the staged Q block lies inside the prefill Q tile: the last prefill item's S MMAs must be done
+                    // the staged Q block lies inside the prefill Q tiles: the last prefill item's S MMAs must be done
                     mbar_wait(BAR(B_QEMPTY), (n_pre & 1) ^ 1);
                     const uint32_t qbytes = (uint32_t)(G * D * 2);
                     mbar_arrive_expect_tx(BAR(B_SCHED_FULL + slot), qbytes);     // release: the record is visible too
@@ -255,12 +306,12 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 if (w.kind == 0) break;
                 const int32_t* bt = prm.block_table + (int64_t)w.req * prm.max_pages;
                 const int g = w.kind == 1 ? w.head / G : w.head;
-                int pg[8];
+                int pg[4];
 #pragma unroll
-                for (int p = 0; p < 8; ++p) pg[p] = nxt_pg[p];
+                for (int p = 0; p < 4; ++p) pg[p] = nxt_pg[p];
                 auto load_pages = [&](int key0) {
 #pragma unroll
-                    for (int p = 0; p < 8; ++p) pg[p] = (key0 + p * kPage < w.kv_end) ? __ldg(bt + (key0 >> 4) + p) : 0;
+                    for (int p = 0; p < 4; ++p) pg[p] = (key0 + p * kPage < w.kv_end) ? __ldg(bt + (key0 >> 4) + p) : 0;
                 };
                 if (w.kind == 1) {
                     mbar_wait(BAR(B_QEMPTY), (n_pre & 1) ^ 1);
@@ -269,49 +320,51 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         const uint32_t pn = n_sched - 2;
                         mbar_wait(BAR(B_SCHED_EMPTY + pn % kSchedSlots), (pn / kSchedSlots) & 1);
                     }
-                    mbar_arrive_expect_tx(BAR(B_QFULL), (uint32_t)SM::kTile);
+                    mbar_arrive_expect_tx(BAR(B_QFULL), (uint32_t)(w.nheads * SM::kQTile));
+                    for (int x = 0; x < w.nheads; ++x)
 #pragma unroll
-                    for (int hh = 0; hh < kHalves; ++hh)
-                        tma_load_2d(sbase + SM::kQOff + hh * (kTileRows * 128), &tmap_q, w.head * D + hh * 64, w.row0, BAR(B_QFULL));
+                        for (int hh = 0; hh < kHalves; ++hh)
+                            tma_load_2d(sbase + SM::kQOff + x * SM::kQTile + hh * (kTileRows * 128), &tmap_q,
+                                        (w.head + x) * D + hh * 64, w.row0, BAR(B_QFULL));
                     ++n_pre;
                 }
                 prev_kind = w.kind;
-                for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kTileKeys, ++tile_ctr) {
-                    if (key0 + kTileKeys >= w.kv_end) {
+                for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kSlotKeys, ++tile_ctr) {
+                    if (key0 + kSlotKeys >= w.kv_end) {
                         // last tile of this item: draw the next ticket now (not earlier, or the tail of the launch
                         // grows by an item held while this one is still streaming); the ring hides the chain
                         fetch(nxt);
                         first_pages(nxt.it, nxt_pg);
                     }
                     const int s = tile_ctr % kNumSt;
-                    const int npages = min(8, (w.kv_end - key0 + kPage - 1) / kPage);
+                    const int npages = min(4, (w.kv_end - key0 + kPage - 1) / kPage);
                     const uint32_t bytes = (uint32_t)npages * kHalves * 2048;
-                    int crow[8];
+                    int crow[4];
 #pragma unroll
-                    for (int p = 0; p < 8; ++p) crow[p] = (pg[p] * Hkv + g) * kPage;
-                    if (key0 + kTileKeys < w.kv_end) load_pages(key0 + kTileKeys);      // next tile's page ids in flight
+                    for (int p = 0; p < 4; ++p) crow[p] = (pg[p] * Hkv + g) * kPage;
+                    if (key0 + kSlotKeys < w.kv_end) load_pages(key0 + kSlotKeys);      // next tile's page ids in flight
                     const uint32_t lt = (lastT >> (2 * s)) & 3u;
                     const uint32_t epar = ((lt == 1 ? parP : parD) >> s) & 1u;
                     // ---- K ----
                     if (lt) mbar_wait(BAR((lt == 1 ? B_KEMPTY_P : B_KEMPTY_D) + s), epar);
                     mbar_arrive_expect_tx(BAR(B_KFULL + s), bytes);
 #pragma unroll
-                    for (int p = 0; p < 8; ++p)
+                    for (int p = 0; p < 4; ++p)
                         if (p < npages) {
 #pragma unroll
                             for (int hh = 0; hh < kHalves; ++hh)
-                                tma_load_2d(sbase + SM::kKOff + s * SM::kTile + hh * (kTileKeys * 128) + p * (kPage * 128),
+                                tma_load_2d(sbase + SM::kKOff + s * SM::kSlot + hh * (kSlotKeys * 128) + p * (kPage * 128),
                                             &tmap_k, hh * 64, crow[p], BAR(B_KFULL + s));
                         }
                     // ---- V ----
                     if (lt) mbar_wait(BAR((lt == 1 ? B_VEMPTY_P : B_VEMPTY_D) + s), epar);
                     mbar_arrive_expect_tx(BAR(B_VFULL + s), bytes);
 #pragma unroll
-                    for (int p = 0; p < 8; ++p)
+                    for (int p = 0; p < 4; ++p)
                         if (p < npages) {
 #pragma unroll
                             for (int hh = 0; hh < kHalves; ++hh)
-                                tma_load_2d(sbase + SM::kVOff + s * SM::kTile + hh * (kTileKeys * 128) + p * (kPage * 128),
+                                tma_load_2d(sbase + SM::kVOff + s * SM::kSlot + hh * (kSlotKeys * 128) + p * (kPage * 128),
                                             &tmap_v, hh * 64, crow[p], BAR(B_VFULL + s));
                         }
                     if (lt == 1) parP ^= 1u << s; else if (lt == 2) parD ^= 1u << s;
@@ -328,65 +381,372 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 }
             }
         }
-    } else if (warp == 1) {
+      } else if (warp == 1) {
         // =============================== tcgen05.mma issuer ===============================
         // Prefill items: one elected thread issues every MMA of the item (waits included), so descriptors stay in
-        // uniform registers.  Decode items: this warp is idle on the data path, so it runs a5 for the workers: it
-        // publishes each split partial (acq_rel ticket) and merges the splits of a (request, kv head) when it draws
-        // the last ticket - off the workers' critical path.
-        constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kTileKeys, 0);
+        // uniform registers.  Decode items: nothing to do here (a5 runs on WG2).
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kSlotKeys, 0);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileRows, D, 1);
-        uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_pre = 0;
+        uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0;
+        uint32_t s_ctr[2] = {0, 0}, n_chain[2] = {0, 0};     // per chain: half tiles / items served so far
         for (;;) {
             const int slot = n_sched % kSchedSlots;
             mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
             const ss_work_item w = sched[slot];
             const int kind = w.kind;
-            const int ntiles = (w.kv_end - w.kv_begin + kTileKeys - 1) / kTileKeys;
+            const int n = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
             ++n_sched;
             if (kind == 0) break;
             if (kind == 1) {
+                const int nq = w.nheads;
                 if (elect_one()) {
-                    const uint64_t qdesc0 = umma_desc_sw128(sbase + SM::kQOff, 16, 1024);
-                    auto issue_s = [&](uint32_t tc, uint32_t sc) {
+                    auto issue_s = [&](int X, int kt) {
+                        const uint32_t tc = tile_ctr + kt, sc = s_ctr[X] + kt;
                         const int s = tc % kNumSt, b = sc & 1;
                         mbar_wait(BAR(B_KFULL + s), (tc / kNumSt) & 1);
                         tc_fence_after();
-                        const uint64_t kdesc0 = umma_desc_sw128(sbase + SM::kKOff + s * SM::kTile, 16, 1024);
+                        const uint64_t qdesc0 = umma_desc_sw128(sbase + SM::kQOff + X * SM::kQTile, 16, 1024);
+                        const uint64_t kdesc0 = umma_desc_sw128(sbase + SM::kKOff + s * SM::kSlot, 16, 1024);
 #pragma unroll
                         for (int ks = 0; ks < D / 16; ++ks) {
-                            const uint32_t off = (ks >> 2) * (kTileRows * 128) + (ks & 3) * 32;      // bytes; descriptor address unit = 16 B
-                            umma_ss(tmem_base + b * 128, qdesc0 + (off >> 4), kdesc0 + (off >> 4), idesc_qk, ks > 0);
+                            // bytes; descriptor address unit = 16 B.  64-column halves: Q 128 rows, K 64 rows apart
+                            const uint32_t qoff = (ks >> 2) * (kTileRows * 128) + (ks & 3) * 32;
+                            const uint32_t koff = (ks >> 2) * (kSlotKeys * 128) + (ks & 3) * 32;
+                            umma_ss(tmem_base + X * SM::kTmemChain + b * 64, qdesc0 + (qoff >> 4), kdesc0 + (koff >> 4), idesc_qk, ks > 0);
                         }
-                        umma_commit(BAR(B_KEMPTY_P + s));
-                        umma_commit(BAR(B_SFULL + b));
+                        umma_commit(BAR(B_SFULL + X * 2 + b));
+                        if (X == nq - 1) umma_commit(BAR(B_KEMPTY_P + s));
                     };
-                    mbar_wait(BAR(B_QFULL), n_pre & 1);
-                    issue_s(tile_ctr, s_ctr);
-                    for (int t = 0; t < ntiles; ++t) {
-                        if (t + 1 < ntiles) issue_s(tile_ctr + t + 1, s_ctr + t + 1);
-                        if (t + 1 == ntiles) umma_commit(BAR(B_QEMPTY));                    // all S MMAs of the item issued
-                        const uint32_t sc = s_ctr + t, tc = tile_ctr + t;
-                        const int b = sc & 1, s = tc % kNumSt;
-                        mbar_wait(BAR(B_PFULL + b), (sc >> 1) & 1);
-                        if (t == 0) mbar_wait(BAR(B_OFREE), (n_pre & 1) ^ 1);               // previous epilogue drained O
+                    auto issue_pv = [&](int X, int kt) {
+                        const uint32_t tc = tile_ctr + kt, sc = s_ctr[X] + kt;
+                        const int s = tc % kNumSt, b = sc & 1;
+                        mbar_wait(BAR(B_PFULL + X * 2 + b), (sc >> 1) & 1);
+                        if (kt == 0) mbar_wait(BAR(B_OFREE + X), (n_chain[X] & 1) ^ 1);     // previous epilogue drained O
                         mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
                         tc_fence_after();
-                        const uint64_t vdesc0 = umma_desc_sw128(sbase + SM::kVOff + s * SM::kTile, kTileKeys * 128, 1024);
+                        const uint64_t vdesc0 = umma_desc_sw128(sbase + SM::kVOff + s * SM::kSlot, kSlotKeys * 128, 1024);
+                        const uint32_t tchain = tmem_base + X * SM::kTmemChain;
 #pragma unroll
-                        for (int kk = 0; kk < kTileKeys / 16; ++kk)      // A = P[b] from TMEM: 16 keys = 8 packed columns
-                            umma_ts(tmem_o, tmem_p + b * 64 + kk * 8, vdesc0 + (uint64_t)(kk * 2048 >> 4), idesc_pv, (t > 0 || kk > 0));
-                        umma_commit(BAR(B_VEMPTY_P + s));
-                        umma_commit(BAR(B_PVDONE));
-                        if (t == ntiles - 1) umma_commit(BAR(B_OFULL));
-                    }
+                        for (int kk = 0; kk < kSlotKeys / 16; ++kk)      // A = P[b] from TMEM: 16 keys = 8 packed columns
+                            umma_ts(tchain + SM::kTmemO, tchain + b * 64 + kk * 8, vdesc0 + (uint64_t)(kk * 2048 >> 4), idesc_pv, (kt > 0 || kk > 0));
+                        umma_commit(BAR(B_PVDONE + X));
+                        if (X == nq - 1) umma_commit(BAR(B_VEMPTY_P + s));
+                        if (kt == n - 1) umma_commit(BAR(B_OFULL + X));
+                    };
+                    mbar_wait(BAR(B_QFULL), n_pre & 1);
+                    for (int kt = 0; kt < 2 && kt < n; ++kt)
+                        for (int X = 0; X < nq; ++X) issue_s(X, kt);
+                    if (n <= 2) umma_commit(BAR(B_QEMPTY));                        // all S MMAs of the item issued
+                    for (int kt = 0; kt < n; ++kt)
+                        for (int X = 0; X < nq; ++X) {
+                            issue_pv(X, kt);
+                            if (kt + 2 < n) {
+                                issue_s(X, kt + 2);
+                                if (kt + 2 == n - 1 && X == nq - 1) umma_commit(BAR(B_QEMPTY));
+                            }
+                        }
                 }
                 __syncwarp();
-                s_ctr += ntiles;
+                for (int X = 0; X < nq; ++X) { s_ctr[X] += n; ++n_chain[X]; }
                 ++n_pre;
-            } else if (w.nsplit > 1) {
-                // ---- a5: publish this split; the last ticket of (request, kv head) merges in fixed split order ----
-                mbar_wait(BAR(B_PARTIAL + slot), ((n_sched - 1) / kSchedSlots) & 1);   // acquire (CTA): all 128 workers' partial stores
+            }
+            tile_ctr += n;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
+        }
+        if (trace && lane == 0) trace[4] = globaltimer_ns();
+      }
+    } else {
+        setmaxnreg_inc<kRegsWorker>();
+        // =============================== workers ===============================
+        const int wg = (warp - 4) >> 2;                        // 0: chain A / decode, 1: chain B / a5 merge
+        const int cw = (warp - 4) & 3;                         // decode: key slice
+        const int quarter = warp & 3;                          // TMEM lane quarter this warp may access
+        const int row = quarter * 32 + lane;                   // prefill: query row inside the tile
+        const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
+        const int wtid = threadIdx.x - 128 - wg * 128;         // 0..127 inside the warpgroup
+        const float sl2 = prm.scale * kMLog2e;
+        const int qrow = lane >> 2, qcol = (lane & 3) * 2;     // mma.sync fragment coordinates
+        const uint32_t tchain = tmem_base + wg * SM::kTmemChain;
+        const uint32_t tmem_o = tchain + SM::kTmemO;
+        uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_chain = 0;
+        float* merge = reinterpret_cast<float*>(smem + SM::kQOff);
+        const bool q_staged = G <= 8;
+        const int mrows = q_staged ? 8 : kMaxGroup;           // merge-buffer rows per warp
+        for (;;) {
+            const int slot = n_sched % kSchedSlots;
+            mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
+            const ss_work_item w = sched[slot];
+            ++n_sched;
+            if (w.kind == 0) break;
+            const int n = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
+            unsigned long long* const tr = (trace && wg == 0 && wtid == 0 && 6 + 9 * (int)n_sched <= prm.trace_words) ? trace + 6 + 9 * (n_sched - 1) : nullptr;
+            if (tr) {
+                tr[0] = globaltimer_ns();
+                tr[2] = ((unsigned long long)w.kind << 32) | (unsigned)n;
+            }
+            if (w.kind == 1 && wg < w.nheads) {
+                // -------------------------- prefill tile, chain wg: thread = query row --------------------------
+                const int u = __ldg(prm.ctx_lens + w.req);
+                const int limit = u + w.q_pos0 + row + 1;            // keys [0, limit) visible to this row
+                const int limit_w = u + w.q_pos0 + quarter * 32 + 1;  // ... to the first row of this warp (the fewest)
+                const int head = w.head + wg;
+                float m = -INFINITY, l = 0.f;
+                for (int kt = 0; kt < n; ++kt) {
+                    const uint32_t sc = s_ctr + kt, tc = tile_ctr + kt;
+                    const int b = sc & 1, s = tc % kNumSt;
+                    const int key0 = kt * kSlotKeys;
+                    const bool tail = key0 + kSlotKeys > w.kv_end;
+                    if (tail) {
+                        // zero V rows [kv_end - key0, 64): stale / unused-slot bits must not meet P = 0 in the MMA
+                        // (both chains write the same zeros; each fences before its own P arrive)
+                        mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
+                        const uint32_t vaddr = sbase + SM::kVOff + s * SM::kSlot;
+                        const int first = w.kv_end - key0;
+                        for (int i = wtid; i < (kSlotKeys - first) * kHalves * 8; i += 128) {
+                            const int r = first + i / (kHalves * 8);
+                            const int c = i % (kHalves * 8);
+                            const uint32_t a = vaddr + (c >> 3) * (kSlotKeys * 128) + r * 128 + (c & 7) * 16;
+                            asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+                        }
+                    }
+                    mbar_wait(BAR(B_SFULL + wg * 2 + b), (sc >> 1) & 1);
+                    tc_fence_after();
+                    if (tr && kt == 0) tr[3] = globaltimer_ns();
+                    uint32_t sr[2][32];
+                    tmem_ld_32x32b_x32(tchain + b * 64 + lane_addr, sr[0]);
+                    tmem_ld_32x32b_x32(tchain + b * 64 + lane_addr + 32, sr[1]);
+                    tmem_ld_wait();
+                    uint32_t pk[32];
+                    float alpha;
+                    if (limit_w - key0 >= kSlotKeys && !tail)       // warp-uniform: every row of this warp sees all 64 keys
+                        alpha = softmax_half<false>(sr, kSlotKeys, sl2, m, l, pk);
+                    else
+                        alpha = softmax_half<true>(sr, min(limit, w.kv_end) - key0, sl2, m, l, pk);
+                    tmem_st_32x32b_x32(tchain + b * 64 + lane_addr, pk);        // P in place over S
+                    if (kt > 0 && !__all_sync(0xffffffffu, alpha == 1.f)) {
+                        mbar_wait(BAR(B_PVDONE + wg), (sc - 1) & 1);          // PV(kt-1) must have landed in O
+                        tc_fence_after();
+#pragma unroll
+                        for (int c = 0; c < D / 32; ++c) {
+                            uint32_t orr[32];
+                            tmem_ld_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
+                            tmem_ld_wait();
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) orr[i] = __float_as_uint(__uint_as_float(orr[i]) * alpha);
+                            tmem_st_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
+                        }
+                    }
+                    tmem_st_wait();
+                    tc_fence_before();
+                    if (tail) fence_proxy_async();   // zeroed V rows -> visible to the MMA's async proxy
+                    mbar_arrive(BAR(B_PFULL + wg * 2 + b));
+                }
+                // ---- epilogue ----
+                if (tr) tr[4] = globaltimer_ns();
+                mbar_wait(BAR(B_OFULL + wg), n_chain & 1);
+                tc_fence_after();
+                const float inv = 1.f / l;
+                const bool store = row < w.nrows;
+                __nv_bfloat16* orow = prm.out + ((int64_t)(w.row0 + row) * Hq + head) * D;
+#pragma unroll
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t orr[32];
+                    tmem_ld_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
+                    tmem_ld_wait();
+                    if (store) {
+#pragma unroll
+                        for (int v = 0; v < 4; ++v) {
+                            uint4 o4;
+                            o4.x = pack_bf16(__uint_as_float(orr[v * 8 + 0]) * inv, __uint_as_float(orr[v * 8 + 1]) * inv);
+                            o4.y = pack_bf16(__uint_as_float(orr[v * 8 + 2]) * inv, __uint_as_float(orr[v * 8 + 3]) * inv);
+                            o4.z = pack_bf16(__uint_as_float(orr[v * 8 + 4]) * inv, __uint_as_float(orr[v * 8 + 5]) * inv);
+                            o4.w = pack_bf16(__uint_as_float(orr[v * 8 + 6]) * inv, __uint_as_float(orr[v * 8 + 7]) * inv);
+                            *reinterpret_cast<uint4*>(orow + c * 32 + v * 8) = o4;
+                        }
+                    }
+                }
+                if (store && prm.lse) prm.lse[(int64_t)(w.row0 + row) * Hq + head] = (m + log2f(l)) * kMLn2;
+                tc_fence_before();
+                mbar_arrive(BAR(B_OFREE + wg));
+                if (wg == 0) mbar_arrive(BAR(B_PARTIAL + slot));    // keeps the per-slot phase count in step (decode-only use)
+                s_ctr += n;
+                ++n_chain;
+            } else if (w.kind == 1) {
+                // single-head item: chain B has nothing to do
+            } else if (wg == 0) {
+                // -------------------------- decode split: warp = 32-key slice of a pair of 64-key slots --------------------------
+                uint32_t qa[D / 16][4];
+                if (q_staged) {
+                    const uint32_t qs = sbase + SM::kQStageOff + slot * SM::kQStageBytes + (qrow * D + qcol) * 2;
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        qa[ks][0] = qrow < G ? lds32(qs + ks * 32) : 0u;
+                        qa[ks][2] = qrow < G ? lds32(qs + ks * 32 + 16) : 0u;
+                        qa[ks][1] = 0u;
+                        qa[ks][3] = 0u;
+                    }
+                } else {
+                    const __nv_bfloat16* qb = prm.q + ((int64_t)w.row0 * Hq + (int64_t)w.head * G) * D;
+#pragma unroll
+                    for (int ks = 0; ks < D / 16; ++ks) {
+                        const int d0 = ks * 16 + qcol;
+                        qa[ks][0] = qrow < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)qrow * D + d0) : 0u;
+                        qa[ks][1] = qrow + 8 < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)(qrow + 8) * D + d0) : 0u;
+                        qa[ks][2] = qrow < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)qrow * D + d0 + 8) : 0u;
+                        qa[ks][3] = qrow + 8 < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)(qrow + 8) * D + d0 + 8) : 0u;
+                    }
+                }
+                float o[D / 8][4];
+#pragma unroll
+                for (int i = 0; i < D / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
+                float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+                const int sub = cw >> 1, r32 = (cw & 1) * 32;      // which slot of the pair, which 32 rows of it
+                for (int t = sub; t < n; t += 2) {
+                    const uint32_t tc = tile_ctr + t;
+                    const int s = tc % kNumSt;
+                    const uint32_t fpar = (tc / kNumSt) & 1;
+                    const int key0 = w.kv_begin + t * kSlotKeys;
+                    const int nvalid = w.kv_end - (key0 + r32);
+                    const uint32_t kbase = sbase + SM::kKOff + s * SM::kSlot;
+                    const uint32_t vbase = sbase + SM::kVOff + s * SM::kSlot;
+                    float sacc[4][4];
+                    mbar_wait(BAR(B_KFULL + s), fpar);
+                    if (tr && t == 0) tr[3] = globaltimer_ns();
+                    if (nvalid > 0) {
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt) sacc[nt][0] = sacc[nt][1] = sacc[nt][2] = sacc[nt][3] = 0.f;
+#pragma unroll
+                        for (int j = 0; j < D / 32; ++j) {
+#pragma unroll
+                            for (int nt = 0; nt < 4; ++nt) {
+                                const int r = r32 + nt * 8 + (lane & 7);
+                                const int cd = 4 * j + (lane >> 3);
+                                const uint32_t a = kbase + (cd >> 3) * (kSlotKeys * 128) + r * 128 + (((cd & 7) ^ (r & 7)) << 4);
+                                uint32_t b0, b1, b2, b3;
+                                ldmatrix_x4(b0, b1, b2, b3, a);
+                                mma_bf16_16816(sacc[nt], qa[2 * j], b0, b1);
+                                mma_bf16_16816(sacc[nt], qa[2 * j + 1], b2, b3);
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(BAR(B_KEMPTY_D + s));
+                    mbar_wait(BAR(B_VFULL + s), fpar);
+                    if (nvalid > 0) {
+                        if (nvalid < 32) {
+                            for (int i = lane; i < (32 - nvalid) * kHalves * 8; i += 32) {
+                                const int r = r32 + nvalid + i / (kHalves * 8);
+                                const int c = i % (kHalves * 8);
+                                const uint32_t a = vbase + (c >> 3) * (kSlotKeys * 128) + r * 128 + (c & 7) * 16;
+                                asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+                            }
+                            __syncwarp();
+                        }
+                        float bm0 = -INFINITY, bm1 = -INFINITY;
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt) {
+                            const int c = nt * 8 + qcol;
+                            if (c >= nvalid) { sacc[nt][0] = -INFINITY; sacc[nt][2] = -INFINITY; }
+                            if (c + 1 >= nvalid) { sacc[nt][1] = -INFINITY; sacc[nt][3] = -INFINITY; }
+                            bm0 = fmaxf(bm0, fmaxf(sacc[nt][0], sacc[nt][1]));
+                            bm1 = fmaxf(bm1, fmaxf(sacc[nt][2], sacc[nt][3]));
+                        }
+                        bm0 = fmaxf(bm0, __shfl_xor_sync(0xffffffffu, bm0, 1));
+                        bm0 = fmaxf(bm0, __shfl_xor_sync(0xffffffffu, bm0, 2));
+                        bm1 = fmaxf(bm1, __shfl_xor_sync(0xffffffffu, bm1, 1));
+                        bm1 = fmaxf(bm1, __shfl_xor_sync(0xffffffffu, bm1, 2));
+                        const float mn0 = fmaxf(m0, bm0 * sl2), mn1 = fmaxf(m1, bm1 * sl2);
+                        const float al0 = exp2f(m0 - mn0), al1 = exp2f(m1 - mn1);
+                        float ps0 = 0.f, ps1 = 0.f;
+                        uint32_t pa[2][4];
+#pragma unroll
+                        for (int nt = 0; nt < 4; ++nt) {
+                            const float p0 = exp2f(sacc[nt][0] * sl2 - mn0), p1 = exp2f(sacc[nt][1] * sl2 - mn0);
+                            const float p2 = exp2f(sacc[nt][2] * sl2 - mn1), p3 = exp2f(sacc[nt][3] * sl2 - mn1);
+                            ps0 += p0 + p1;
+                            ps1 += p2 + p3;
+                            pa[nt >> 1][(nt & 1) * 2 + 0] = pack_bf16(p0, p1);
+                            pa[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2, p3);
+                        }
+                        l0 = l0 * al0 + ps0;
+                        l1 = l1 * al1 + ps1;
+                        m0 = mn0;
+                        m1 = mn1;
+#pragma unroll
+                        for (int i = 0; i < D / 8; ++i) { o[i][0] *= al0; o[i][1] *= al0; o[i][2] *= al1; o[i][3] *= al1; }
+#pragma unroll
+                        for (int kk = 0; kk < 2; ++kk) {
+#pragma unroll
+                            for (int np = 0; np < D / 16; ++np) {
+                                const int r = r32 + kk * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
+                                const int cd = 2 * np + (lane >> 4);
+                                const uint32_t a = vbase + (cd >> 3) * (kSlotKeys * 128) + r * 128 + (((cd & 7) ^ (r & 7)) << 4);
+                                uint32_t b0, b1, b2, b3;
+                                ldmatrix_x4_trans(b0, b1, b2, b3, a);
+                                mma_bf16_16816(o[2 * np], pa[kk], b0, b1);
+                                mma_bf16_16816(o[2 * np + 1], pa[kk], b2, b3);
+                            }
+                        }
+                        if (nvalid < 32) fence_proxy_async();
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(BAR(B_VEMPTY_D + s));
+                }
+                // ---- cross-warp log-sum-exp merge through smem ----
+                if (tr) tr[4] = globaltimer_ns();
+                l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
+                l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+                l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
+                l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+                float* mine = merge + cw * mrows * (D + 2);
+#pragma unroll
+                for (int i = 0; i < D / 8; ++i) {
+                    *reinterpret_cast<float2*>(mine + qrow * (D + 2) + i * 8 + qcol) = make_float2(o[i][0], o[i][1]);
+                    if (!q_staged) *reinterpret_cast<float2*>(mine + (qrow + 8) * (D + 2) + i * 8 + qcol) = make_float2(o[i][2], o[i][3]);
+                }
+                if ((lane & 3) == 0) {
+                    mine[qrow * (D + 2) + D] = m0;
+                    mine[qrow * (D + 2) + D + 1] = l0;
+                    if (!q_staged) {
+                        mine[(qrow + 8) * (D + 2) + D] = m1;
+                        mine[(qrow + 8) * (D + 2) + D + 1] = l1;
+                    }
+                }
+                named_bar_sync(1, 128);
+                if (tr) tr[5] = globaltimer_ns();
+                for (int e = wtid; e < G * D; e += 128) {
+                    const int r = e / D, d = e % D;
+                    float M = -INFINITY;
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) M = fmaxf(M, merge[(x * mrows + r) * (D + 2) + D]);
+                    float L = 0.f, acc = 0.f;
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) {
+                        const float* src = merge + (x * mrows + r) * (D + 2);
+                        const float wgt = exp2f(src[D] - M);           // a warp that saw no key: m = -inf -> weight 0
+                        L += src[D + 1] * wgt;
+                        acc += src[d] * wgt;
+                    }
+                    if (w.nsplit == 1) {
+                        const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r;
+                        prm.out[orow * D + d] = __float2bfloat16_rn(acc / L);
+                        if (prm.lse && d == 0) prm.lse[orow] = (M + log2f(L)) * kMLn2;
+                    } else {
+                        float* dst = prm.partials + ((int64_t)(w.partial + w.split) * G + r) * (D + 2);
+                        dst[d] = acc;
+                        if (d == 0) { dst[D] = M; dst[D + 1] = L; }
+                    }
+                }
+                if (tr) tr[6] = globaltimer_ns();
+                // a5 hand-off: WG2 publishes this split and, if it was the last of its (request, kv head), merges all
+                // of them; the decode warps go straight on to the next item.  mbarrier arrive = release at CTA scope
+                // for this thread's partial stores.
+                mbar_arrive(BAR(B_PARTIAL + slot));           // once per item and slot use (phase = slot use count)
+                named_bar_sync(1, 128);                       // merge buffer free for the next item
+            } else if (cw == 0 && w.nsplit > 1) {
+                // ---- a5 (WG2 warp 0): publish this split; the last ticket of (request, kv head) merges in fixed split order ----
+                mbar_wait(BAR(B_PARTIAL + slot), ((n_sched - 1) / kSchedSlots) & 1);   // acquire (CTA): all 128 decode threads' partial stores
                 int last = 0;
                 if (lane == 0) last = atom_add_acq_rel_gpu(prm.merge_counters + w.req * Hkv + w.head, 1) == w.nsplit - 1;
                 last = __shfl_sync(0xffffffffu, last, 0);
@@ -441,325 +801,12 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     if (lane == 0) prm.merge_counters[w.req * Hkv + w.head] = 0;     // re-armed for the next call
                 }
             }
-            tile_ctr += ntiles;
-            __syncwarp();
-            if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
-        }
-        if (trace && lane == 0) trace[4] = globaltimer_ns();
-    } else {
-        // =============================== workers ===============================
-        const int cw = warp - 2;                               // decode: key slice; also == TMEM lane quarter order below
-        const int quarter = warp & 3;                          // TMEM lane quarter this warp may access
-        const int row = quarter * 32 + lane;                   // prefill: query row inside the tile
-        const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
-        const int wtid = threadIdx.x - 64;                     // 0..127
-        const float sl2 = prm.scale * kMLog2e;
-        const int qrow = lane >> 2, qcol = (lane & 3) * 2;     // mma.sync fragment coordinates
-        uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_pre = 0;
-        float* merge = reinterpret_cast<float*>(smem + SM::kQOff);
-        int* flag = reinterpret_cast<int*>(smem + SM::kTmemSlotOff + 16);
-        const bool q_staged = G <= 8;
-        const int mrows = q_staged ? 8 : kMaxGroup;           // merge-buffer rows per warp
-        for (;;) {
-            const int slot = n_sched % kSchedSlots;
-            mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
-            const ss_work_item w = sched[slot];
-            ++n_sched;
-            if (w.kind == 0) break;
-            const int ntiles = (w.kv_end - w.kv_begin + kTileKeys - 1) / kTileKeys;
-            unsigned long long* const tr = (trace && wtid == 0 && 6 + 9 * (int)n_sched <= prm.trace_words) ? trace + 6 + 9 * (n_sched - 1) : nullptr;
-            if (tr) {
-                tr[0] = globaltimer_ns();
-                tr[2] = ((unsigned long long)w.kind << 32) | (unsigned)ntiles;
-            }
-            if (w.kind == 1) {
-                // -------------------------- prefill tile: thread = query row --------------------------
-                const int u = __ldg(prm.ctx_lens + w.req);
-                const int limit = u + w.q_pos0 + row + 1;            // keys [0, limit) visible to this row
-                float m = -INFINITY, l = 0.f;
-                for (int t = 0; t < ntiles; ++t) {
-                    const uint32_t sc = s_ctr + t, tc = tile_ctr + t;
-                    const int b = sc & 1, s = tc % kNumSt;
-                    const int key0 = t * kTileKeys;
-                    if (key0 + kTileKeys > w.kv_end) {
-                        // zero V rows [kv_end - key0, 128): stale / unused-slot bits must not meet P = 0 in the MMA
-                        mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
-                        const uint32_t vaddr = sbase + SM::kVOff + s * SM::kTile;
-                        const int first = w.kv_end - key0;
-                        for (int i = wtid; i < (kTileKeys - first) * kHalves * 8; i += 128) {
-                            const int r = first + i / (kHalves * 8);
-                            const int c = i % (kHalves * 8);
-                            const uint32_t a = vaddr + (c >> 3) * (kTileKeys * 128) + r * 128 + (c & 7) * 16;
-                            asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
-                        }
-                    }
-                    mbar_wait(BAR(B_SFULL + b), (sc >> 1) & 1);
-                    tc_fence_after();
-                    if (tr && t == 0) tr[3] = globaltimer_ns();
-                    uint32_t sr[4][32];
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) tmem_ld_32x32b_x32(tmem_base + b * 128 + lane_addr + c * 32, sr[c]);
-                    tmem_ld_wait();
-                    const int nvis = limit - key0;
-                    float bm = -INFINITY;
-                    if (nvis >= kTileKeys) {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c)
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) bm = fmaxf(bm, __uint_as_float(sr[c][i]));
-                    } else {
-#pragma unroll
-                        for (int c = 0; c < 4; ++c)
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) {
-                                if (c * 32 + i >= nvis) sr[c][i] = 0xff800000u;   // -inf by select, never by arithmetic
-                                bm = fmaxf(bm, __uint_as_float(sr[c][i]));
-                            }
-                    }
-                    // lazy rescale: only move the reference max when it grows by more than 2^8
-                    const float cand = bm * sl2;
-                    float m_new = m, alpha = 1.f;
-                    if (cand > m + kRescaleThreshold) { m_new = cand; alpha = exp2f(m - m_new); }   // tile 0: m = -inf -> alpha = 0
-                    float psum = 0.f;
-                    // P = exp2(s*sl2 - m_new) -> bf16 pairs -> TMEM (A operand of the PV MMA), 64 packed columns per row
-#pragma unroll
-                    for (int hh = 0; hh < 2; ++hh) {
-                        uint32_t pk[32];
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) {
-                            const float p0 = exp2f(__uint_as_float(sr[2 * hh + (i >> 4)][(2 * i) & 31]) * sl2 - m_new);
-                            const float p1 = exp2f(__uint_as_float(sr[2 * hh + (i >> 4)][((2 * i) & 31) + 1]) * sl2 - m_new);
-                            psum += p0 + p1;
-                            pk[i] = pack_bf16(p0, p1);
-                        }
-                        tmem_st_32x32b_x32(tmem_p + b * 64 + lane_addr + hh * 32, pk);
-                    }
-                    l = l * alpha + psum;
-                    m = m_new;
-                    if (t > 0 && !__all_sync(0xffffffffu, alpha == 1.f)) {
-                        mbar_wait(BAR(B_PVDONE), (sc - 1) & 1);          // PV(t-1) must have landed in O
-                        tc_fence_after();
-#pragma unroll
-                        for (int c = 0; c < D / 32; ++c) {
-                            uint32_t orr[32];
-                            tmem_ld_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
-                            tmem_ld_wait();
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) orr[i] = __float_as_uint(__uint_as_float(orr[i]) * alpha);
-                            tmem_st_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
-                        }
-                    }
-                    tmem_st_wait();
-                    tc_fence_before();
-                    if (key0 + kTileKeys > w.kv_end) fence_proxy_async();   // zeroed V rows -> visible to the MMA's async proxy
-                    mbar_arrive(BAR(B_PFULL + b));
-                }
-                // ---- epilogue ----
-                if (tr) tr[4] = globaltimer_ns();
-                mbar_wait(BAR(B_OFULL), n_pre & 1);
-                tc_fence_after();
-                const float inv = 1.f / l;
-                const bool store = row < w.nrows;
-                __nv_bfloat16* orow = prm.out + ((int64_t)(w.row0 + row) * Hq + w.head) * D;
-#pragma unroll
-                for (int c = 0; c < D / 32; ++c) {
-                    uint32_t orr[32];
-                    tmem_ld_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
-                    tmem_ld_wait();
-                    if (store) {
-#pragma unroll
-                        for (int v = 0; v < 4; ++v) {
-                            uint4 pk;
-                            pk.x = pack_bf16(__uint_as_float(orr[v * 8 + 0]) * inv, __uint_as_float(orr[v * 8 + 1]) * inv);
-                            pk.y = pack_bf16(__uint_as_float(orr[v * 8 + 2]) * inv, __uint_as_float(orr[v * 8 + 3]) * inv);
-                            pk.z = pack_bf16(__uint_as_float(orr[v * 8 + 4]) * inv, __uint_as_float(orr[v * 8 + 5]) * inv);
-                            pk.w = pack_bf16(__uint_as_float(orr[v * 8 + 6]) * inv, __uint_as_float(orr[v * 8 + 7]) * inv);
-                            *reinterpret_cast<uint4*>(orow + c * 32 + v * 8) = pk;
-                        }
-                    }
-                }
-                if (store && prm.lse) prm.lse[(int64_t)(w.row0 + row) * Hq + w.head] = (m + log2f(l)) * kMLn2;
-                tc_fence_before();
-                mbar_arrive(BAR(B_OFREE));
-                mbar_arrive(BAR(B_PARTIAL + slot));               // keeps the per-slot phase count in step (decode-only use)
-                s_ctr += ntiles;
-                ++n_pre;
-            } else {
-                // -------------------------- decode split: warp = 32-key slice --------------------------
-                uint32_t qa[D / 16][4];
-                if (q_staged) {
-                    const uint32_t qs = sbase + SM::kQStageOff + slot * SM::kQStageBytes + (qrow * D + qcol) * 2;
-#pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks) {
-                        qa[ks][0] = qrow < G ? lds32(qs + ks * 32) : 0u;
-                        qa[ks][2] = qrow < G ? lds32(qs + ks * 32 + 16) : 0u;
-                        qa[ks][1] = 0u;
-                        qa[ks][3] = 0u;
-                    }
-                } else {
-                    const __nv_bfloat16* qb = prm.q + ((int64_t)w.row0 * Hq + (int64_t)w.head * G) * D;
-#pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks) {
-                        const int d0 = ks * 16 + qcol;
-                        qa[ks][0] = qrow < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)qrow * D + d0) : 0u;
-                        qa[ks][1] = qrow + 8 < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)(qrow + 8) * D + d0) : 0u;
-                        qa[ks][2] = qrow < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)qrow * D + d0 + 8) : 0u;
-                        qa[ks][3] = qrow + 8 < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)(qrow + 8) * D + d0 + 8) : 0u;
-                    }
-                }
-                float o[D / 8][4];
-#pragma unroll
-                for (int i = 0; i < D / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
-                float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
-                for (int t = 0; t < ntiles; ++t) {
-                    const uint32_t tc = tile_ctr + t;
-                    const int s = tc % kNumSt;
-                    const uint32_t fpar = (tc / kNumSt) & 1;
-                    const int key0 = w.kv_begin + t * kTileKeys;
-                    const int nvalid = w.kv_end - (key0 + 32 * cw);
-                    const uint32_t kbase = sbase + SM::kKOff + s * SM::kTile;
-                    const uint32_t vbase = sbase + SM::kVOff + s * SM::kTile;
-                    float sacc[4][4];
-                    mbar_wait(BAR(B_KFULL + s), fpar);
-                    if (tr && t == 0) tr[3] = globaltimer_ns();
-                    if (nvalid > 0) {
-#pragma unroll
-                        for (int nt = 0; nt < 4; ++nt) sacc[nt][0] = sacc[nt][1] = sacc[nt][2] = sacc[nt][3] = 0.f;
-#pragma unroll
-                        for (int j = 0; j < D / 32; ++j) {
-#pragma unroll
-                            for (int nt = 0; nt < 4; ++nt) {
-                                const int r = 32 * cw + nt * 8 + (lane & 7);
-                                const int cd = 4 * j + (lane >> 3);
-                                const uint32_t a = kbase + (cd >> 3) * (kTileKeys * 128) + r * 128 + (((cd & 7) ^ (r & 7)) << 4);
-                                uint32_t b0, b1, b2, b3;
-                                ldmatrix_x4(b0, b1, b2, b3, a);
-                                mma_bf16_16816(sacc[nt], qa[2 * j], b0, b1);
-                                mma_bf16_16816(sacc[nt], qa[2 * j + 1], b2, b3);
-                            }
-                        }
-                    }
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(BAR(B_KEMPTY_D + s));
-                    mbar_wait(BAR(B_VFULL + s), fpar);
-                    if (nvalid > 0) {
-                        if (nvalid < 32) {
-                            for (int i = lane; i < (32 - nvalid) * kHalves * 8; i += 32) {
-                                const int r = 32 * cw + nvalid + i / (kHalves * 8);
-                                const int c = i % (kHalves * 8);
-                                const uint32_t a = vbase + (c >> 3) * (kTileKeys * 128) + r * 128 + (c & 7) * 16;
-                                asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
-                            }
-                            __syncwarp();
-                        }
-                        float bm0 = -INFINITY, bm1 = -INFINITY;
-#pragma unroll
-                        for (int nt = 0; nt < 4; ++nt) {
-                            const int c = nt * 8 + qcol;
-                            if (c >= nvalid) { sacc[nt][0] = -INFINITY; sacc[nt][2] = -INFINITY; }
-                            if (c + 1 >= nvalid) { sacc[nt][1] = -INFINITY; sacc[nt][3] = -INFINITY; }
-                            bm0 = fmaxf(bm0, fmaxf(sacc[nt][0], sacc[nt][1]));
-                            bm1 = fmaxf(bm1, fmaxf(sacc[nt][2], sacc[nt][3]));
-                        }
-                        bm0 = fmaxf(bm0, __shfl_xor_sync(0xffffffffu, bm0, 1));
-                        bm0 = fmaxf(bm0, __shfl_xor_sync(0xffffffffu, bm0, 2));
-                        bm1 = fmaxf(bm1, __shfl_xor_sync(0xffffffffu, bm1, 1));
-                        bm1 = fmaxf(bm1, __shfl_xor_sync(0xffffffffu, bm1, 2));
-                        const float mn0 = fmaxf(m0, bm0 * sl2), mn1 = fmaxf(m1, bm1 * sl2);
-                        const float al0 = exp2f(m0 - mn0), al1 = exp2f(m1 - mn1);
-                        float ps0 = 0.f, ps1 = 0.f;
-                        uint32_t pa[2][4];
-#pragma unroll
-                        for (int nt = 0; nt < 4; ++nt) {
-                            const float p0 = exp2f(sacc[nt][0] * sl2 - mn0), p1 = exp2f(sacc[nt][1] * sl2 - mn0);
-                            const float p2 = exp2f(sacc[nt][2] * sl2 - mn1), p3 = exp2f(sacc[nt][3] * sl2 - mn1);
-                            ps0 += p0 + p1;
-                            ps1 += p2 + p3;
-                            pa[nt >> 1][(nt & 1) * 2 + 0] = pack_bf16(p0, p1);
-                            pa[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2, p3);
-                        }
-                        l0 = l0 * al0 + ps0;
-                        l1 = l1 * al1 + ps1;
-                        m0 = mn0;
-                        m1 = mn1;
-#pragma unroll
-                        for (int i = 0; i < D / 8; ++i) { o[i][0] *= al0; o[i][1] *= al0; o[i][2] *= al1; o[i][3] *= al1; }
-#pragma unroll
-                        for (int kk = 0; kk < 2; ++kk) {
-#pragma unroll
-                            for (int np = 0; np < D / 16; ++np) {
-                                const int r = 32 * cw + kk * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
-                                const int cd = 2 * np + (lane >> 4);
-                                const uint32_t a = vbase + (cd >> 3) * (kTileKeys * 128) + r * 128 + (((cd & 7) ^ (r & 7)) << 4);
-                                uint32_t b0, b1, b2, b3;
-                                ldmatrix_x4_trans(b0, b1, b2, b3, a);
-                                mma_bf16_16816(o[2 * np], pa[kk], b0, b1);
-                                mma_bf16_16816(o[2 * np + 1], pa[kk], b2, b3);
-                            }
-                        }
-                        if (nvalid < 32) fence_proxy_async();
-                    }
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(BAR(B_VEMPTY_D + s));
-                }
-                // ---- cross-warp log-sum-exp merge through smem ----
-                if (tr) tr[4] = globaltimer_ns();
-                l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
-                l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
-                l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
-                l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
-                float* mine = merge + cw * mrows * (D + 2);
-#pragma unroll
-                for (int i = 0; i < D / 8; ++i) {
-                    *reinterpret_cast<float2*>(mine + qrow * (D + 2) + i * 8 + qcol) = make_float2(o[i][0], o[i][1]);
-                    if (!q_staged) *reinterpret_cast<float2*>(mine + (qrow + 8) * (D + 2) + i * 8 + qcol) = make_float2(o[i][2], o[i][3]);
-                }
-                if ((lane & 3) == 0) {
-                    mine[qrow * (D + 2) + D] = m0;
-                    mine[qrow * (D + 2) + D + 1] = l0;
-                    if (!q_staged) {
-                        mine[(qrow + 8) * (D + 2) + D] = m1;
-                        mine[(qrow + 8) * (D + 2) + D + 1] = l1;
-                    }
-                }
-                named_bar_sync(1, 128);
-                if (tr) tr[5] = globaltimer_ns();
-                for (int e = wtid; e < G * D; e += 128) {
-                    const int r = e / D, d = e % D;
-                    float M = -INFINITY;
-#pragma unroll
-                    for (int x = 0; x < 4; ++x) M = fmaxf(M, merge[(x * mrows + r) * (D + 2) + D]);
-                    float L = 0.f, acc = 0.f;
-#pragma unroll
-                    for (int x = 0; x < 4; ++x) {
-                        const float* src = merge + (x * mrows + r) * (D + 2);
-                        const float wgt = exp2f(src[D] - M);
-                        L += src[D + 1] * wgt;
-                        acc += src[d] * wgt;
-                    }
-                    if (w.nsplit == 1) {
-                        const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r;
-                        prm.out[orow * D + d] = __float2bfloat16_rn(acc / L);
-                        if (prm.lse && d == 0) prm.lse[orow] = (M + log2f(L)) * kMLn2;
-                    } else {
-                        float* dst = prm.partials + ((int64_t)(w.partial + w.split) * G + r) * (D + 2);
-                        dst[d] = acc;
-                        if (d == 0) { dst[D] = M; dst[D + 1] = L; }
-                    }
-                }
-                if (tr) tr[6] = globaltimer_ns();
-                // a5 hand-off: the (otherwise idle) MMA warp publishes this split and, if it was the last of its
-                // (request, kv head), merges all of them; the workers go straight on to the next item.  mbarrier
-                // arrive = release at CTA scope for this thread's partial stores.
-                mbar_arrive(BAR(B_PARTIAL + slot));           // once per item and slot use (phase = slot use count)
-                named_bar_sync(1, 128);                       // merge buffer free for the next item
-            }
-            tile_ctr += ntiles;
+            tile_ctr += n;
             if (tr) tr[1] = globaltimer_ns();
             __syncwarp();
             if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
         }
-        if (trace && wtid == 0) { trace[2] = globaltimer_ns(); trace[3] = n_sched - 1; }
+        if (trace && wg == 0 && wtid == 0) { trace[2] = globaltimer_ns(); trace[3] = n_sched - 1; }
     }
 
     // ---- teardown ----

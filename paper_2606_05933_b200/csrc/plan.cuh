@@ -1,7 +1,9 @@
 // a2 work-list plan (SURVEY.md §8(a) "work-list build"; north_star (d)): partitions the ragged batch {(c_r, u_r)}
 // into CTA-sized work items from query_start_loc and ctx_lens only.
 //   c_r == 0 -> nothing;  c_r == 1 -> decode set D;  c_r > 1 -> prefill set P   (Eq. 2)
-//   prefill: one item per (request, 128-row tile, query head), keys [0, u + last row + 1), heaviest tile first
+//   prefill: one item per (request, 128-row tile, PAIR of query heads of one kv head), keys [0, u + last row + 1),
+//            heaviest tile first.  The two heads share every staged K/V tile and run as two independent softmax
+//            chains (attn_mixed.cu); a group with an odd number of heads (G = 1, 7) ends in a single-head item
 //   decode : one item per (request, KV split, kv head); the split length L is chosen so that the batch yields
 //            ~kDecodeWaves items per SM (tile aligned, clamped to [kMinSplitKeys, kMaxSplitKeys])
 // Requests of each kind are ranked heavy-first (longest KV range first) so the tail of the persistent main kernel
@@ -32,6 +34,9 @@ struct PlanTables {
 };
 
 __device__ __forceinline__ int plan_ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+// prefill items per (request, row tile): Hkv groups x ceil(G / 2) head pairs
+__host__ __device__ __forceinline__ int plan_head_pairs(int Hq, int Hkv) { return Hkv * ((Hq / Hkv + 1) / 2); }
 
 // balanced split of n keys into ceil(n / L) tile-aligned chunks
 __device__ __forceinline__ int plan_decode_chunk(int n, int L) {
@@ -147,7 +152,7 @@ __device__ void build_plan(const int32_t* __restrict__ qsl, const int32_t* __res
             carry += __shfl_sync(0xffffffffu, incl, 31);
         }
         if (lane == 0) {
-            const int tot_p = tiles_p * Hq, tot_d = carry * Hkv;
+            const int tot_p = tiles_p * plan_head_pairs(Hq, Hkv), tot_d = carry * Hkv;
             ph->tot_p = tot_p;
             ph->tot_d = tot_d;
             // SM partition between the two queues: SM-time of the decode items at the per-SM streaming rate vs SM-time
@@ -177,17 +182,19 @@ __device__ __forceinline__ void plan_decode_item(int idx, const PlanHeader* ph, 
                                                  int Hq, int Hkv, ss_work_item& it) {
     const int nP = ph->nP;
     if (idx < ph->tot_p) {
-        const int unit = idx / Hq;
+        const int G = Hq / Hkv, GP = (G + 1) / 2, HP = Hkv * GP;
+        const int unit = idx / HP;
         int lo = 0, hi = nP;                             // last k with off[k] <= unit
         while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if ((int)tb.off[mid] <= unit) lo = mid; else hi = mid; }
-        const int r = tb.ord[lo], local = idx - (int)tb.off[lo] * Hq;
+        const int r = tb.ord[lo], local = idx - (int)tb.off[lo] * HP;
         const int q0 = __ldg(qsl + r), c = __ldg(qsl + r + 1) - q0, u = __ldg(ctx_lens + r);
         const int ntile = plan_ceil_div(c, kTileRows);
-        const int mt = ntile - 1 - local / Hq;           // heaviest (last) tile first
+        const int mt = ntile - 1 - local / HP;           // heaviest (last) tile first
         const int nrows = min(kTileRows, c - mt * kTileRows);
-        it.kind = 1; it.req = r; it.head = local % Hq; it.row0 = q0 + mt * kTileRows; it.nrows = nrows;
+        const int hp = local % HP, g = hp / GP, j = hp % GP;
+        it.kind = 1; it.req = r; it.head = g * G + 2 * j; it.row0 = q0 + mt * kTileRows; it.nrows = nrows;
         it.kv_begin = 0; it.kv_end = u + mt * kTileRows + nrows; it.split = 0; it.nsplit = 1;
-        it.partial = -1; it.q_pos0 = mt * kTileRows; it.reserved = 0;
+        it.partial = -1; it.q_pos0 = mt * kTileRows; it.nheads = (2 * j + 1 < G) ? 2 : 1;
     } else {
         const int didx = idx - ph->tot_p, unit = didx / Hkv;
         int lo = 0, hi = ph->nD;
@@ -199,7 +206,7 @@ __device__ __forceinline__ void plan_decode_item(int idx, const PlanHeader* ph, 
         it.kind = 2; it.req = r; it.head = g; it.row0 = __ldg(qsl + r); it.nrows = 1;
         it.kv_begin = s * chunk; it.kv_end = min(n, (s + 1) * chunk); it.split = s; it.nsplit = ns;
         it.partial = ns > 1 ? base + g * ns : -1;        // partial slots share the decode items' index space
-        it.q_pos0 = 0; it.reserved = 0;
+        it.q_pos0 = 0; it.nheads = Hq / Hkv;
     }
 }
 

@@ -290,7 +290,8 @@ def test_worklist_partitions_the_batch():
         c, u = b.reqs[it["req"]]
         assert c > 1 and it["kv_end"] == u + it["q_pos0"] + it["nrows"] and it["kv_begin"] == 0
         assert it["row0"] == b.query_start_loc[it["req"]] + it["q_pos0"] and 1 <= it["nrows"] <= 128
-        covered[it["row0"]:it["row0"] + it["nrows"], it["head"]] += 1
+        assert it["nheads"] in (1, 2) and it["head"] // 8 == (it["head"] + it["nheads"] - 1) // 8    # one KV group
+        covered[it["row0"]:it["row0"] + it["nrows"], it["head"]:it["head"] + it["nheads"]] += 1
     spans = {}
     for it in dec:
         c, u = b.reqs[it["req"]]
@@ -313,10 +314,9 @@ def test_worklist_partitions_the_batch():
     assert len(slots) <= n_part          # partial slots share the decode items' index space
     assert (covered == 1).all()
     # heavy-first inside each kind: prefill requests by KV length (u + c), and inside a request the last (heaviest)
-    # row tile first; the 64 heads of one (request, row tile) are consecutive
-    first_head = pre[::64]
-    assert (pre["head"].reshape(-1, 64) == np.arange(64)).all()
-    big = [r for r in np.unique(first_head["req"])]
+    # row tile first; the 32 head pairs of one (request, row tile) are consecutive
+    first_head = pre[::32]
+    assert (pre["head"].reshape(-1, 32) == 2 * np.arange(32)).all() and (pre["nheads"] == 2).all()
     req_order = list(dict.fromkeys(int(r) for r in first_head["req"]))
     kv_len = [b.reqs[r][0] + b.reqs[r][1] for r in req_order]
     assert kv_len == sorted(kv_len, reverse=True)
