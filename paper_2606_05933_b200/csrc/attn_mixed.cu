@@ -4,7 +4,7 @@
 // Persistent CTAs (one per SM) pull items from the device work list through a dynamic queue (atomic
 // counter), so tensor-bound prefill tiles and HBM-bound decode splits overlap across SMs and the batch
 // costs ~max(bytes/HBM, flops/tensor) instead of the sum.  12 warps per CTA in 3 warpgroups; the register
-// file is re-partitioned with setmaxnreg (WG0 80 registers per thread, WG1 / WG2 216):
+// file is re-partitioned with setmaxnreg (WG0 72 registers per thread, WG1 / WG2 216):
 //   WG0 warp 0  scheduler + TMA producer (one elected thread).  Publishes each item to the other warps through a
 //               4-slot smem ring, loads the Q tiles (prefill: the item's 1 or 2 query heads, 128 rows each) and
 //               streams 64-key K and V tiles — 4 pages x D/64 boxes of 16 rows x 128 B, SWIZZLE_128B — into
@@ -42,7 +42,10 @@ constexpr int kMixThreads = 384;
 constexpr int kSlotKeys = 64;        // keys per K / V ring slot = keys per S buffer
 constexpr int kNumSt = 5;            // K ring slots = V ring slots
 constexpr int kSchedSlots = 4;
-constexpr int kRegsWg0 = 80, kRegsWorker = 216;      // 128*80 + 256*216 = 65536
+// setmaxnreg moves registers inside the CTA's own launch allocation: 384 threads x 168 (the __launch_bounds__ cap ptxas
+// reports) = 64512, so 128*72 + 256*216 = 64512 fits exactly; one register more per worker and the .inc spins forever.
+constexpr int kRegsLaunch = 168, kRegsWg0 = 72, kRegsWorker = 216;
+static_assert(128 * kRegsWg0 + 256 * kRegsWorker <= kMixThreads * kRegsLaunch, "setmaxnreg.inc could never be granted");
 constexpr float kMLog2e = 1.4426950408889634f;
 constexpr float kMLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.f;   // log2 units: P <= 2^8, safe in bf16 / fp32
@@ -180,9 +183,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             mbar_init(BAR(B_KFULL + s), 1);
             mbar_init(BAR(B_VFULL + s), 1);
             mbar_init(BAR(B_KEMPTY_P + s), 1);
-            mbar_init(BAR(B_KEMPTY_D + s), 2);
+            mbar_init(BAR(B_KEMPTY_D + s), 4);
             mbar_init(BAR(B_VEMPTY_P + s), 1);
-            mbar_init(BAR(B_VEMPTY_D + s), 2);
+            mbar_init(BAR(B_VEMPTY_D + s), 4);
         }
         for (int b = 0; b < 4; ++b) {
             mbar_init(BAR(B_SFULL + b), 1);
@@ -601,13 +604,16 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
 #pragma unroll
                 for (int i = 0; i < D / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
                 float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+                // Warps 0,1 compute on the even slots of the item, warps 2,3 on the odd ones (32 rows each), but EVERY warp
+                // waits FULL and arrives EMPTY on EVERY slot: an mbarrier parity wait is only sound while the waiter is
+                // less than one phase away from the barrier, and with 5 ring slots a slot alternates between the pairs.
                 const int sub = cw >> 1, r32 = (cw & 1) * 32;      // which slot of the pair, which 32 rows of it
-                for (int t = sub; t < n; t += 2) {
+                for (int t = 0; t < n; ++t) {
                     const uint32_t tc = tile_ctr + t;
                     const int s = tc % kNumSt;
                     const uint32_t fpar = (tc / kNumSt) & 1;
                     const int key0 = w.kv_begin + t * kSlotKeys;
-                    const int nvalid = w.kv_end - (key0 + r32);
+                    const int nvalid = (t & 1) == sub ? w.kv_end - (key0 + r32) : 0;      // 0: not this warp's slot
                     const uint32_t kbase = sbase + SM::kKOff + s * SM::kSlot;
                     const uint32_t vbase = sbase + SM::kVOff + s * SM::kSlot;
                     float sacc[4][4];

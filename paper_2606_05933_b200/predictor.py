@@ -5,10 +5,21 @@ Model (Eq. 5, index read as j = 1..7, reading 13):  T_hat
 the 7 features of Table 1, a global model trained on all samples and a scene expert model
 (pure decode / pure prefill / mixed, Eq. 3) for every scene with at least `min_expert_samples`
 samples; inference uses the expert if one exists, else the global model.  The paper names the
-threshold but gives no value: 12 here (reading 15).  Fit = ordinary least squares (the paper says
-"lightweight ... linear"; no regulariser is mentioned), features scaled to unit max for conditioning only.
+threshold but gives no value: 12 here (reading 15).
 
-    python -m paper_2606_05933_b200.predictor profiles/r1_v4_surface.csv profiles/r1_v4_surface_dense.csv
+Fit.  The paper says only "lightweight ... linear"; no regulariser or constraint is mentioned.  Two fits are offered:
+  "ols"   ordinary least squares (round 1): best in-sample error, but on a small surface it takes negative weights on
+          x6 / x7, so T_hat is NOT monotone in the token budget;
+  "nnls"  (default) least squares with a free intercept and NON-NEGATIVE weights on the basis
+          (x1 - x2/2, x2, x3, ..., x7) (Lawson-Hanson via scipy.optimize.nnls), mapped back to weights on x1..x7, so
+          the model is still Eq. 5's linear form; the only weight that may be negative is w2 >= -w1/2.  Why this
+          basis: a causal chunk visits c*u + c(c+1)/2 = x1 - x2/2 + x6/2 (row, key) pairs, so the physical weight
+          of x2 IS negative; every basis element is a count of work that is non-decreasing in the token budget
+          (d/dc [c(u+c) - c^2/2] = u + c >= 0), hence Pred(b) is non-decreasing in b, which TimeToBudget's binary
+          search needs (reading 16).
+Features are scaled to unit max for conditioning only.
+
+    python -m paper_2606_05933_b200.predictor [--shape 32/8/128] [--fit nnls|ols] surface.csv [more.csv ...]
 
 prints MAE / RMSE / R^2 the way Table 5 does, in-sample and leave-one-out.
 """
@@ -25,17 +36,35 @@ SCENES = ["pure_decode", "pure_prefill", "mixed"]
 
 
 class LinearLatencyModel:
-    """T_hat = b + w . x  (Eq. 5), least squares."""
+    """T_hat = b + w . x  (Eq. 5), least squares; fit = "nnls" (w >= 0, intercept free) or "ols"."""
 
-    def __init__(self):
+    def __init__(self, fit: str = "nnls"):
+        if fit not in ("nnls", "ols"):
+            raise ValueError(fit)
+        self.fit_mode = fit
         self.scale: Optional[np.ndarray] = None
         self.coef: Optional[np.ndarray] = None
 
     def fit(self, X: np.ndarray, y: np.ndarray) -> "LinearLatencyModel":
-        X = np.asarray(X, dtype=np.float64)
+        X, y = np.asarray(X, dtype=np.float64), np.asarray(y, dtype=np.float64)
         self.scale = np.maximum(np.abs(X).max(axis=0), 1.0)
-        A = np.hstack([np.ones((X.shape[0], 1)), X / self.scale])
-        self.coef, *_ = np.linalg.lstsq(A, np.asarray(y, dtype=np.float64), rcond=None)
+        Xs = X / self.scale
+        if self.fit_mode == "ols":
+            A = np.hstack([np.ones((X.shape[0], 1)), Xs])
+            self.coef, *_ = np.linalg.lstsq(A, y, rcond=None)
+        else:
+            from scipy.optimize import nnls
+            # basis z = (x1 - x2/2, x2, x3..x7) in scaled units; free intercept = difference of two non-negative
+            # columns (+1, -1); a >= 0 on the basis, then w1 = a1, w2 = a2 - a1/2 (in unscaled units)
+            Z = X.copy()
+            Z[:, 0] = X[:, 0] - 0.5 * X[:, 1]
+            zs = np.maximum(np.abs(Z).max(axis=0), 1.0)
+            A = np.hstack([np.ones((X.shape[0], 1)), -np.ones((X.shape[0], 1)), Z / zs])
+            z, _ = nnls(A, y, maxiter=50 * A.shape[1])
+            a = z[2:] / zs                                   # unscaled basis weights
+            w = a.copy()
+            w[1] = a[1] - 0.5 * a[0]
+            self.coef = np.concatenate([[z[0] - z[1]], w * self.scale])
         return self
 
     def predict(self, X: np.ndarray) -> np.ndarray:
@@ -54,9 +83,10 @@ class LinearLatencyModel:
 class BatchLatencyPredictor:
     """Global model + scene experts."""
 
-    def __init__(self, min_expert_samples: int = 12):
+    def __init__(self, min_expert_samples: int = 12, fit: str = "nnls"):
         self.min_expert_samples = min_expert_samples
-        self.global_model = LinearLatencyModel()
+        self.fit_mode = fit
+        self.global_model = LinearLatencyModel(fit)
         self.experts: Dict[str, LinearLatencyModel] = {}
 
     def fit(self, X: np.ndarray, y: np.ndarray, scenes: Sequence[str]) -> "BatchLatencyPredictor":
@@ -66,7 +96,7 @@ class BatchLatencyPredictor:
         for sc in SCENES:
             idx = scenes == sc
             if int(idx.sum()) >= self.min_expert_samples:
-                self.experts[sc] = LinearLatencyModel().fit(X[idx], y[idx])
+                self.experts[sc] = LinearLatencyModel(self.fit_mode).fit(X[idx], y[idx])
         return self
 
     def predict(self, X: np.ndarray, scenes: Sequence[str]) -> np.ndarray:
@@ -95,12 +125,12 @@ def load_surface(path):
     return rows, X, y, scenes, shapes
 
 
-def evaluate(path: str, shape: str = "32/8/128", min_expert_samples: int = 12) -> Dict[str, Dict[str, float]]:
+def evaluate(path, shape: str = "32/8/128", min_expert_samples: int = 12, fit: str = "nnls") -> Dict[str, Dict[str, float]]:
     """In-sample and leave-one-out fidelity on the points of one layer shape (latency depends on the shape)."""
     rows, X, y, scenes, shapes = load_surface(path)
     keep = [i for i, s in enumerate(shapes) if s == shape]
     X, y, scenes = X[keep], y[keep], [scenes[i] for i in keep]
-    p = BatchLatencyPredictor(min_expert_samples).fit(X, y, scenes)
+    p = BatchLatencyPredictor(min_expert_samples, fit).fit(X, y, scenes)
     res = {"n": {"points": len(keep), **{sc: scenes.count(sc) for sc in SCENES}},
            "experts": {sc: 1.0 for sc in p.experts},
            "in_sample": scores(y, p.predict(X, scenes)),
@@ -109,23 +139,31 @@ def evaluate(path: str, shape: str = "32/8/128", min_expert_samples: int = 12) -
     for i in range(len(y)):
         m = np.ones(len(y), dtype=bool)
         m[i] = False
-        q = BatchLatencyPredictor(min_expert_samples).fit(X[m], y[m], [s for s, k in zip(scenes, m) if k])
+        q = BatchLatencyPredictor(min_expert_samples, fit).fit(X[m], y[m], [s for s, k in zip(scenes, m) if k])
         loo[i] = q.predict(X[i:i + 1], [scenes[i]])[0]
     res["leave_one_out"] = scores(y, loo)
     res["mean_latency_us"] = {"value": float(y.mean())}
+    res["weights"] = {sc: {"intercept": m.intercept, **{f: float(w) for f, w in zip(FEATURES, m.weights)}}
+                      for sc, m in [("global", p.global_model), *p.experts.items()]}
     return res
 
 
 def main(argv: Optional[List[str]] = None):
-    argv = sys.argv[1:] if argv is None else argv
-    path = argv if argv else ["profiles/r1_v4_surface.csv", "profiles/r1_v4_surface_dense.csv"]
-    res = evaluate(path)
-    print(f"surface: {path}  points (8B shape): {res['n']}")
+    import argparse
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--shape", default="32/8/128")
+    ap.add_argument("--fit", default="nnls", choices=["nnls", "ols"])
+    ap.add_argument("csv", nargs="+")
+    args = ap.parse_args(argv)
+    res = evaluate(args.csv, shape=args.shape, fit=args.fit)
+    print(f"surface: {args.csv}  shape {args.shape}  fit {args.fit}  points: {res['n']}")
     print(f"experts trained for: {sorted(res['experts'])}")
     for k in ("in_sample", "global_only_in_sample", "leave_one_out"):
         r = res[k]
         print(f"{k:24s} MAE {r['mae']:.2f} us  RMSE {r['rmse']:.2f} us  R^2 {r['r2']:.4f}")
     print(f"mean latency {res['mean_latency_us']['value']:.1f} us")
+    for sc, w in res["weights"].items():
+        print(f"weights[{sc}]: " + "  ".join(f"{k}={v:.4g}" for k, v in w.items()))
 
 
 if __name__ == "__main__":

@@ -42,8 +42,32 @@ def dense_points() -> List[tuple]:
     return pts
 
 
-def surface_points(with_c4: bool = False, dense: bool = False) -> List[tuple]:
+def model_points(model: str) -> List[tuple]:
+    """The same grid on another layer shape (one predictor model set per shape: latency depends on Hq/Hkv/D)."""
+    Hq, Hkv, D = wl.MODEL_SHAPES[model]
+    pts = []
+    for nd in (32, 128):
+        for C in (256, 512, 1024, 2048):
+            for n in (1, 2, 4):
+                pts.append((f"{model}/C3:{C},{n},{nd}", lambda C=C, n=n, nd=nd: wl.config_c3(C, n, nd, model=model)))
+    for med in (500, 4000):
+        for nd in (32, 128):
+            for C in (0, 1024):
+                pts.append((f"{model}/CTX:{C},1,{nd},m{med}", lambda C=C, nd=nd, med=med: wl.config_c3(C, 1, nd, ctx_median=med, model=model)))
+    for nd in (16, 32, 64, 128, 192):
+        pts.append((f"{model}/PD-{nd}", lambda nd=nd: wl.config_c3(0, 1, nd, model=model)))
+    for i, (c, u) in enumerate([(256, 0), (512, 2048), (1024, 0), (1024, 4096), (2048, 0), (2048, 4096), (2048, 8192), (4096, 0),
+                                (128, 1024), (768, 512), (1536, 3000), (384, 6000)]):
+        pts.append((f"{model}/PP:{c},{u}", lambda c=c, u=u, i=i: wl.make_batch(f"PP-{model}-{c}-{u}", Hq, Hkv, D, [(c, u)], 7200 + i)))
+    for i, rs in enumerate([[(512, 0), (512, 3000)], [(1024, 0), (1024, 6000)], [(256, 100), (256, 2000), (256, 4000), (256, 8000)]]):
+        pts.append((f"{model}/PP2:{i}", lambda rs=rs, i=i: wl.make_batch(f"PP2-{model}-{i}", Hq, Hkv, D, rs, 7300 + i)))
+    return pts
+
+
+def surface_points(with_c4: bool = False, dense: bool = False, model: Optional[str] = None) -> List[tuple]:
     """(point id, Batch factory) for the whole grid, in a fixed order."""
+    if model:
+        return model_points(model)
     if dense:
         return dense_points()
     pts = []
@@ -112,6 +136,7 @@ def main(argv=None):
     ap.add_argument("--with-c4", action="store_true", help="include the 40 GB-pool decode-heavy config")
     ap.add_argument("--only", default=None, help="comma-separated point-id prefixes")
     ap.add_argument("--dense", action="store_true", help="the extra between-the-lines points instead of the grid")
+    ap.add_argument("--model", default=None, help="run the grid on another layer shape (workloads.MODEL_SHAPES key)")
     args = ap.parse_args(argv)
     import torch
     if not torch.cuda.is_available():
@@ -123,7 +148,7 @@ def main(argv=None):
     with open(args.out, "w", newline="") as f:
         wr = csv.DictWriter(f, fieldnames=FIELDS)
         wr.writeheader()
-        for pid, make in surface_points(args.with_c4, args.dense):
+        for pid, make in surface_points(args.with_c4, args.dense, args.model):
             if args.only and not any(pid.startswith(p) for p in args.only.split(",")):
                 continue
             b = make()

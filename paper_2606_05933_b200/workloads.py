@@ -102,6 +102,14 @@ def make_batch(name: str, Hq: int, Hkv: int, D: int, reqs: Sequence[Tuple[int, i
 # --------------------------------------------------------------------------------------------
 LOGNORMAL_SIGMA = 0.75       # not given by BASELINE.json; reading stated in DESIGN.md
 
+# Layer shapes (Hq, Hkv, D) of the models the paper serves (PAPER.md:382 "Llama3-8B and Qwen2.5-7B", tensor parallel
+# degree 2 on its 2-GPU boxes), from the public model configs; SURVEY.md section 8(f) NEXT-3.  Qwen2.5-7B has 28 query
+# and 4 KV heads: G = 7, the first non-power-of-two group (TP2 slice: 14/2, also G = 7).
+MODEL_SHAPES = {
+    "llama3-8b": (32, 8, 128), "llama3-70b": (64, 8, 128), "qwen2.5-7b": (28, 4, 128),
+    "llama3-8b-tp2": (16, 4, 128), "qwen2.5-7b-tp2": (14, 2, 128),
+}
+
 
 def _lognormal_ctx(rng, median, size, cap):
     return np.clip(np.rint(rng.lognormal(math.log(median), LOGNORMAL_SIGMA, size=size)), 1, cap
@@ -126,18 +134,24 @@ def c3_split(C: int, n: int) -> List[int]:
     return [C // n + (1 if i < C % n else 0) for i in range(n)]
 
 
-def config_c3(C: int, n: int, N_d: int, ctx_median: int = 1500, shuffle: bool = False) -> Batch:
+def config_c3(C: int, n: int, N_d: int, ctx_median: int = 1500, shuffle: bool = False,
+              model: str = "llama3-8b") -> Batch:
     """C3 grid point: chunk budget C over n prefill requests (ctx U{0..4096}) + N_d decodes
-    (ctx lognormal, median 1500 unless swept, cap 8192).  C may be 0 (pure decode)."""
+    (ctx lognormal, median 1500 unless swept, cap 8192).  C may be 0 (pure decode).  `model` picks the layer shape
+    (BASELINE.json configs[2] is the Llama-3-8B shape; the other shapes reuse the recipe with their own seeds)."""
     seed = 3000 + (100 if N_d == 128 else 0) + (10 * int(round(math.log2(C / 256))) if C > 0 else 90) + n
     if ctx_median != 1500:
         seed += 7 * ctx_median
+    if model != "llama3-8b":
+        seed += 100000 * (1 + sorted(MODEL_SHAPES).index(model))
+    Hq, Hkv, D = MODEL_SHAPES[model]
     rng = np.random.default_rng(seed)
     pu = rng.integers(0, 4096, size=n, endpoint=True)
     du = _lognormal_ctx(rng, ctx_median, N_d, 8192)
     reqs = ([(c, int(u)) for c, u in zip(c3_split(C, n), pu)] if C > 0 else []) + \
            [(1, int(u)) for u in du]
-    return make_batch(f"C3-C{C}-n{n}-Nd{N_d}-m{ctx_median}", 32, 8, 128, reqs, seed, rng=rng,
+    tag = "" if model == "llama3-8b" else f"-{model}"
+    return make_batch(f"C3-C{C}-n{n}-Nd{N_d}-m{ctx_median}{tag}", Hq, Hkv, D, reqs, seed, rng=rng,
                       shuffle_requests=shuffle,
                       meta={"chunk": C, "n_prefill": n if C > 0 else 0, "n_decode": N_d,
                             "ctx_median": ctx_median})
@@ -171,15 +185,6 @@ def config_c5(seed: int = 5, shuffle: bool = False) -> Batch:
     reqs = [(1024, 0), (1024, 6000)] + [(1, int(u)) for u in dec]
     return make_batch("C5-70B-mixed", 64, 8, 128, reqs, seed, rng=rng, with_append=True,
                       shuffle_requests=shuffle)
-
-
-# Layer shapes (Hq, Hkv, D) of the models the paper serves (PAPER.md:382 "Llama3-8B and Qwen2.5-7B", tensor parallel
-# degree 2 on its 2-GPU boxes), from the public model configs; SURVEY.md section 8(f) NEXT-3.  Qwen2.5-7B has 28 query
-# and 4 KV heads: G = 7, the first non-power-of-two group (TP2 slice: 14/2, also G = 7).
-MODEL_SHAPES = {
-    "llama3-8b": (32, 8, 128), "llama3-70b": (64, 8, 128), "qwen2.5-7b": (28, 4, 128),
-    "llama3-8b-tp2": (16, 4, 128), "qwen2.5-7b-tp2": (14, 2, 128),
-}
 
 
 def config_model_mixed(model: str, seed: int = 6, chunk: int = 512, chunk_ctx: int = 1024, n_decode: int = 64,
