@@ -10,7 +10,8 @@
 //               streams 64-key K and V tiles — 4 pages x D/64 boxes of 16 rows x 128 B, SWIZZLE_128B — into
 //               separate 5-slot K and V rings (a K slot is free as soon as its S MMAs are done, a V slot as soon
 //               as its PV MMAs are done).
-//   WG0 warp 1  tcgen05.mma issuer + TMEM owner (prefill items only), one elected thread.  Per query head X (a
+//   WG0 warps 1,2  tcgen05.mma issuers (warp 1 also owns the TMEM allocation), one elected thread each: warp 1 issues
+//               chain A's MMAs, warp 2 chain B's (prefill items only).  Per query head X (a
 //               "chain") TMEM holds S_X[0], S_X[1] (128 rows x 64 keys fp32, 64 columns each) and O_X (128 x D
 //               fp32): 2 x 256 = all 512 columns.  P (bf16 pairs) is written IN PLACE over its S buffer, so per
 //               chain the order is  S(k) -> softmax -> P(k) -> PV(k) -> S(k+2)  with S(k+1) already done: each
@@ -33,6 +34,17 @@
 #include "common.cuh"
 #include "plan.cuh"
 #include "ptx.cuh"
+
+// -DSS_PROFILE (measurement builds only, see profiles/): clock64 phase counters of the prefill loop, written into the
+// ss_debug_set_trace buffer - per item words 5..8 = chain A's cycles in {S wait, tcgen05.ld, softmax, st + fence +
+// arrive}; the last 4 words of the CTA block = the MMA thread's cycles in {P wait, K/V wait, issue} and its half tiles.
+#ifdef SS_PROFILE
+#define SS_PF(i) { const long long c_ = clock64(); pf_acc[i] += c_ - pf_t; pf_t = c_; }
+#define SS_MM(i) { const long long c_ = clock64(); mm_acc[i] += c_ - mm_t; mm_t = c_; }
+#else
+#define SS_PF(i)
+#define SS_MM(i)
+#endif
 
 namespace ss {
 
@@ -125,6 +137,27 @@ struct MixParams {
     const int32_t* err_flag;       // SS_FLAG_DEBUG_CHECKS: nonzero = the metadata check tripped, serve no item; else null
 };
 
+// exp2 on the FMA / ALU pipes for two values at once (the MUFU pipe does 16 ex2 per clock and SM: at 128 x 64 scores per
+// chain and half tile it alone would take as long as the two MMAs): round-to-nearest split x = n + f, |f| <= 0.5, by
+// the 1.5 * 2^23 magic add; cubic minimax polynomial for 2^f (max relative error 7.6e-5, P is rounded to bf16 = 3.9e-3
+// anyway); 2^n by adding n to the exponent field.  x is clamped at -126 so the result never leaves the normal range.
+__device__ __forceinline__ float2 exp2_poly2(float2 x) {
+    const float kMagic = 12582912.f;                   // 1.5 * 2^23: the integer part lands in the low mantissa bits
+    x.x = fmaxf(x.x, -126.f);
+    x.y = fmaxf(x.y, -126.f);
+    const float2 t = __fadd2_rn(x, make_float2(kMagic, kMagic));
+    const float2 f = __fadd2_rn(x, __ffma2_rn(t, make_float2(-1.f, -1.f), make_float2(kMagic, kMagic)));   // x - round(x)
+    float2 q = __ffma2_rn(f, make_float2(0.055170879f, 0.055170879f), make_float2(0.24260919f, 0.24260919f));
+    q = __ffma2_rn(q, f, make_float2(0.69326097f, 0.69326097f));
+    q = __ffma2_rn(q, f, make_float2(0.99992818f, 0.99992818f));
+    return make_float2(__uint_as_float(__float_as_uint(q.x) + (__float_as_uint(t.x) << 23)),
+                       __uint_as_float(__float_as_uint(q.y) + (__float_as_uint(t.y) << 23)));
+}
+#ifndef SS_POLY_EVERY
+#define SS_POLY_EVERY 3
+#endif
+constexpr int kPolyEvery = SS_POLY_EVERY;      // every kPolyEvery-th pair of scores takes exp2_poly2 instead of MUFU.EX2 (0 = none)
+
 // One 64-key half tile of one query row: S (64 fp32 scores in sr) -> P (bf16 pairs in pk), online-softmax state (m, l).
 // MASKED: keys at and after nvis are invisible (causal diagonal / end of the KV range); replaced by select.
 // Returns alpha (the factor the accumulated O row must be scaled by; 1 unless the reference max moved).
@@ -148,7 +181,7 @@ __device__ __forceinline__ float softmax_half(uint32_t (&sr)[2][32], int nvis, f
 #pragma unroll
     for (int i = 0; i < 32; ++i) {
         const float2 x = __ffma2_rn(make_float2(__uint_as_float(sr[i >> 4][(2 * i) & 31]), __uint_as_float(sr[i >> 4][((2 * i) & 31) + 1])), sl2v, nm);
-        const float2 p = make_float2(exp2f(x.x), exp2f(x.y));
+        const float2 p = (kPolyEvery > 0 && i % (kPolyEvery > 0 ? kPolyEvery : 1) == 0) ? exp2_poly2(x) : make_float2(exp2f(x.x), exp2f(x.y));
         ps[i & 3] = __fadd2_rn(ps[i & 3], p);
         pk[i] = pack_bf16(p.x, p.y);
     }
@@ -182,9 +215,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         for (int s = 0; s < kNumSt; ++s) {
             mbar_init(BAR(B_KFULL + s), 1);
             mbar_init(BAR(B_VFULL + s), 1);
-            mbar_init(BAR(B_KEMPTY_P + s), 1);
+            mbar_init(BAR(B_KEMPTY_P + s), 2);               // one commit per chain
             mbar_init(BAR(B_KEMPTY_D + s), 4);
-            mbar_init(BAR(B_VEMPTY_P + s), 1);
+            mbar_init(BAR(B_VEMPTY_P + s), 2);
             mbar_init(BAR(B_VEMPTY_D + s), 4);
         }
         for (int b = 0; b < 4; ++b) {
@@ -192,7 +225,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             mbar_init(BAR(B_PFULL + b), 128);
         }
         mbar_init(BAR(B_QFULL), 1);
-        mbar_init(BAR(B_QEMPTY), 1);
+        mbar_init(BAR(B_QEMPTY), 2);
         for (int x = 0; x < 2; ++x) {
             mbar_init(BAR(B_OFULL + x), 1);
             mbar_init(BAR(B_OFREE + x), 128);
@@ -201,7 +234,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         for (int s = 0; s < kSchedSlots; ++s) {
             mbar_init(BAR(B_PARTIAL + s), 128);
             mbar_init(BAR(B_SCHED_FULL + s), 1);
-            mbar_init(BAR(B_SCHED_EMPTY + s), 9);                // MMA warp + 8 worker warps
+            mbar_init(BAR(B_SCHED_EMPTY + s), 10);               // 2 MMA warps + 8 worker warps
         }
         fence_barrier_init();
         prefetch_tmap(&tmap_q);
@@ -296,7 +329,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 dst[0] = wu.v[0]; dst[1] = wu.v[1]; dst[2] = wu.v[2];
                 const ss_work_item& w = wu.it;
                 if (w.kind == 2 && q_staged) {
-                    // the staged Q block lies inside the prefill Q tiles: the last prefill item's S MMAs must be done
+                    // the staged Q block lies inside the prefill Q tiles: the last prefill item's MMAs must be done
                     mbar_wait(BAR(B_QEMPTY), (n_pre & 1) ^ 1);
                     const uint32_t qbytes = (uint32_t)(G * D * 2);
                     mbar_arrive_expect_tx(BAR(B_SCHED_FULL + slot), qbytes);     // release: the record is visible too
@@ -384,14 +417,19 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 }
             }
         }
-      } else if (warp == 1) {
-        // =============================== tcgen05.mma issuer ===============================
-        // Prefill items: one elected thread issues every MMA of the item (waits included), so descriptors stay in
-        // uniform registers.  Decode items: nothing to do here (a5 runs on WG2).
+      } else if (warp <= 2) {
+        // =============================== tcgen05.mma issuers ===============================
+        // Warp 1 issues chain A's MMAs, warp 2 chain B's (one elected thread each, waits included, so descriptors stay
+        // in uniform registers).  Two issuers because one thread could not keep the pipe fed: per (chain, half tile)
+        // it spent ~250 cycles in three mbarrier round trips and ~740 blocked in issue (profiles/r2_a3.md), serially
+        // for both chains.  The chains touch disjoint TMEM and only read the shared K/V slots, so no order is needed
+        // between them; the slot / Q-tile release barriers take one commit per chain (chain A commits twice when the
+        // item has a single head).  Decode items: nothing to do here (a5 runs on WG2).
         constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kSlotKeys, 0);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileRows, D, 1);
-        uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0;
-        uint32_t s_ctr[2] = {0, 0}, n_chain[2] = {0, 0};     // per chain: half tiles / items served so far
+        const int X = warp - 1;
+        const uint32_t tchain = tmem_base + X * SM::kTmemChain;
+        uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0, s_ctr = 0, n_chain = 0;   // s_ctr / n_chain: this chain's half tiles / items
         for (;;) {
             const int slot = n_sched % kSchedSlots;
             mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
@@ -402,12 +440,18 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             if (kind == 0) break;
             if (kind == 1) {
                 const int nq = w.nheads;
-                if (elect_one()) {
-                    auto issue_s = [&](int X, int kt) {
-                        const uint32_t tc = tile_ctr + kt, sc = s_ctr[X] + kt;
+                if (X < nq && elect_one()) {
+                    const int ncommit = nq == 1 ? 2 : 1;          // arrivals this chain owes the shared (count 2) barriers
+#ifdef SS_PROFILE
+                    long long mm_t = 0, mm_acc[4] = {0, 0, 0, 0};      // wait P (+O free) | wait K/V | issue | -
+#endif
+                    auto issue_s = [&](int kt) {
+                        const uint32_t tc = tile_ctr + kt, sc = s_ctr + kt;
                         const int s = tc % kNumSt, b = sc & 1;
+                        SS_MM(2)
                         mbar_wait(BAR(B_KFULL + s), (tc / kNumSt) & 1);
                         tc_fence_after();
+                        SS_MM(1)
                         const uint64_t qdesc0 = umma_desc_sw128(sbase + SM::kQOff + X * SM::kQTile, 16, 1024);
                         const uint64_t kdesc0 = umma_desc_sw128(sbase + SM::kKOff + s * SM::kSlot, 16, 1024);
 #pragma unroll
@@ -415,49 +459,62 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                             // bytes; descriptor address unit = 16 B.  64-column halves: Q 128 rows, K 64 rows apart
                             const uint32_t qoff = (ks >> 2) * (kTileRows * 128) + (ks & 3) * 32;
                             const uint32_t koff = (ks >> 2) * (kSlotKeys * 128) + (ks & 3) * 32;
-                            umma_ss(tmem_base + X * SM::kTmemChain + b * 64, qdesc0 + (qoff >> 4), kdesc0 + (koff >> 4), idesc_qk, ks > 0);
+                            umma_ss(tchain + b * 64, qdesc0 + (qoff >> 4), kdesc0 + (koff >> 4), idesc_qk, ks > 0);
                         }
                         umma_commit(BAR(B_SFULL + X * 2 + b));
-                        if (X == nq - 1) umma_commit(BAR(B_KEMPTY_P + s));
+                        for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_KEMPTY_P + s));
                     };
-                    auto issue_pv = [&](int X, int kt) {
-                        const uint32_t tc = tile_ctr + kt, sc = s_ctr[X] + kt;
+                    auto issue_pv = [&](int kt) {
+                        const uint32_t tc = tile_ctr + kt, sc = s_ctr + kt;
                         const int s = tc % kNumSt, b = sc & 1;
+                        SS_MM(2)
                         mbar_wait(BAR(B_PFULL + X * 2 + b), (sc >> 1) & 1);
-                        if (kt == 0) mbar_wait(BAR(B_OFREE + X), (n_chain[X] & 1) ^ 1);     // previous epilogue drained O
+                        if (kt == 0) mbar_wait(BAR(B_OFREE + X), (n_chain & 1) ^ 1);     // previous epilogue drained O
+                        SS_MM(0)
                         mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
                         tc_fence_after();
+                        SS_MM(1)
                         const uint64_t vdesc0 = umma_desc_sw128(sbase + SM::kVOff + s * SM::kSlot, kSlotKeys * 128, 1024);
-                        const uint32_t tchain = tmem_base + X * SM::kTmemChain;
 #pragma unroll
                         for (int kk = 0; kk < kSlotKeys / 16; ++kk)      // A = P[b] from TMEM: 16 keys = 8 packed columns
                             umma_ts(tchain + SM::kTmemO, tchain + b * 64 + kk * 8, vdesc0 + (uint64_t)(kk * 2048 >> 4), idesc_pv, (kt > 0 || kk > 0));
                         umma_commit(BAR(B_PVDONE + X));
-                        if (X == nq - 1) umma_commit(BAR(B_VEMPTY_P + s));
-                        if (kt == n - 1) umma_commit(BAR(B_OFULL + X));
+                        for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_VEMPTY_P + s));
+                        if (kt == n - 1) {
+                            umma_commit(BAR(B_OFULL + X));
+                            // Q tiles free for the next item.  Committed after the LAST MMA of the item (not the last
+                            // S): when the next Q tile lands, every K and V tile issued before it has landed too, so a
+                            // role that sat out an item (chain B on single-head items, both issuers on decode items)
+                            // can never run a parity wait one phase early on a ring slot.
+                            for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_QEMPTY));
+                        }
                     };
                     mbar_wait(BAR(B_QFULL), n_pre & 1);
-                    for (int kt = 0; kt < 2 && kt < n; ++kt)
-                        for (int X = 0; X < nq; ++X) issue_s(X, kt);
-                    if (n <= 2) umma_commit(BAR(B_QEMPTY));                        // all S MMAs of the item issued
-                    for (int kt = 0; kt < n; ++kt)
-                        for (int X = 0; X < nq; ++X) {
-                            issue_pv(X, kt);
-                            if (kt + 2 < n) {
-                                issue_s(X, kt + 2);
-                                if (kt + 2 == n - 1 && X == nq - 1) umma_commit(BAR(B_QEMPTY));
-                            }
-                        }
+#ifdef SS_PROFILE
+                    mm_t = clock64();
+#endif
+                    for (int kt = 0; kt < 2 && kt < n; ++kt) issue_s(kt);
+                    for (int kt = 0; kt < n; ++kt) {
+                        issue_pv(kt);
+                        if (kt + 2 < n) issue_s(kt + 2);
+                    }
+#ifdef SS_PROFILE
+                    SS_MM(2)
+                    if (trace && prm.trace_words >= 16 && X == 0) {
+                        unsigned long long* tw = trace + prm.trace_words - 4;
+                        tw[0] += mm_acc[0]; tw[1] += mm_acc[1]; tw[2] += mm_acc[2]; tw[3] += (unsigned long long)n;
+                    }
+#endif
                 }
                 __syncwarp();
-                for (int X = 0; X < nq; ++X) { s_ctr[X] += n; ++n_chain[X]; }
+                if (X < nq) { s_ctr += n; ++n_chain; }
                 ++n_pre;
             }
             tile_ctr += n;
             __syncwarp();
             if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
         }
-        if (trace && lane == 0) trace[4] = globaltimer_ns();
+        if (trace && lane == 0 && X == 0) trace[4] = globaltimer_ns();
       }
     } else {
         setmaxnreg_inc<kRegsWorker>();
@@ -495,14 +552,21 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 const int limit_w = u + w.q_pos0 + quarter * 32 + 1;  // ... to the first row of this warp (the fewest)
                 const int head = w.head + wg;
                 float m = -INFINITY, l = 0.f;
+#ifdef SS_PROFILE
+                long long pf_t = clock64(), pf_acc[4] = {0, 0, 0, 0};     // S wait | tcgen05.ld | softmax | st + fence + arrive
+#endif
                 for (int kt = 0; kt < n; ++kt) {
                     const uint32_t sc = s_ctr + kt, tc = tile_ctr + kt;
                     const int b = sc & 1, s = tc % kNumSt;
                     const int key0 = kt * kSlotKeys;
                     const bool tail = key0 + kSlotKeys > w.kv_end;
+                    mbar_wait(BAR(B_SFULL + wg * 2 + b), (sc >> 1) & 1);
+                    tc_fence_after();
                     if (tail) {
                         // zero V rows [kv_end - key0, 64): stale / unused-slot bits must not meet P = 0 in the MMA
-                        // (both chains write the same zeros; each fences before its own P arrive)
+                        // (both chains write the same zeros; each fences before its own P arrive).  After the S wait:
+                        // S(kt) done => this item's Q landed => every earlier tile landed (see B_QEMPTY), so the
+                        // V wait below is never a phase early.
                         mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
                         const uint32_t vaddr = sbase + SM::kVOff + s * SM::kSlot;
                         const int first = w.kv_end - key0;
@@ -513,19 +577,20 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                             asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
                         }
                     }
-                    mbar_wait(BAR(B_SFULL + wg * 2 + b), (sc >> 1) & 1);
-                    tc_fence_after();
                     if (tr && kt == 0) tr[3] = globaltimer_ns();
+                    SS_PF(0)
                     uint32_t sr[2][32];
                     tmem_ld_32x32b_x32(tchain + b * 64 + lane_addr, sr[0]);
                     tmem_ld_32x32b_x32(tchain + b * 64 + lane_addr + 32, sr[1]);
                     tmem_ld_wait();
+                    SS_PF(1)
                     uint32_t pk[32];
                     float alpha;
                     if (limit_w - key0 >= kSlotKeys && !tail)       // warp-uniform: every row of this warp sees all 64 keys
                         alpha = softmax_half<false>(sr, kSlotKeys, sl2, m, l, pk);
                     else
                         alpha = softmax_half<true>(sr, min(limit, w.kv_end) - key0, sl2, m, l, pk);
+                    SS_PF(2)
                     tmem_st_32x32b_x32(tchain + b * 64 + lane_addr, pk);        // P in place over S
                     if (kt > 0 && !__all_sync(0xffffffffu, alpha == 1.f)) {
                         mbar_wait(BAR(B_PVDONE + wg), (sc - 1) & 1);          // PV(kt-1) must have landed in O
@@ -544,9 +609,13 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     tc_fence_before();
                     if (tail) fence_proxy_async();   // zeroed V rows -> visible to the MMA's async proxy
                     mbar_arrive(BAR(B_PFULL + wg * 2 + b));
+                    SS_PF(3)
                 }
                 // ---- epilogue ----
                 if (tr) tr[4] = globaltimer_ns();
+#ifdef SS_PROFILE
+                if (tr) { tr[5] = pf_acc[0]; tr[6] = pf_acc[1]; tr[7] = pf_acc[2]; tr[8] = pf_acc[3]; }
+#endif
                 mbar_wait(BAR(B_OFULL + wg), n_chain & 1);
                 tc_fence_after();
                 const float inv = 1.f / l;
