@@ -614,27 +614,36 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 // ---- epilogue ----
                 if (tr) tr[4] = globaltimer_ns();
 #ifdef SS_PROFILE
-                if (tr) { tr[5] = pf_acc[0]; tr[6] = pf_acc[1]; tr[7] = pf_acc[2]; tr[8] = pf_acc[3]; }
+                if (tr) { tr[6] = pf_acc[1]; tr[7] = pf_acc[2]; tr[8] = pf_acc[3]; }
+#endif
+#ifdef SS_PROFILE
+                pf_t = clock64();
 #endif
                 mbar_wait(BAR(B_OFULL + wg), n_chain & 1);
                 tc_fence_after();
+#ifdef SS_PROFILE
+                if (tr) tr[5] = (unsigned long long)pf_acc[0] | ((unsigned long long)(clock64() - pf_t) << 32);
+#endif
                 const float inv = 1.f / l;
                 const bool store = row < w.nrows;
                 __nv_bfloat16* orow = prm.out + ((int64_t)(w.row0 + row) * Hq + head) * D;
+                // thread = row: D fp32 -> D bf16 = 2 D bytes contiguous, written as 32-byte (whole-sector) stores
 #pragma unroll
-                for (int c = 0; c < D / 32; ++c) {
-                    uint32_t orr[32];
-                    tmem_ld_32x32b_x32(tmem_o + lane_addr + c * 32, orr);
+                for (int c = 0; c < D / 64; ++c) {
+                    uint32_t orr[2][32];
+                    tmem_ld_32x32b_x32(tmem_o + lane_addr + c * 64, orr[0]);
+                    tmem_ld_32x32b_x32(tmem_o + lane_addr + c * 64 + 32, orr[1]);
                     tmem_ld_wait();
                     if (store) {
 #pragma unroll
                         for (int v = 0; v < 4; ++v) {
-                            uint4 o4;
-                            o4.x = pack_bf16(__uint_as_float(orr[v * 8 + 0]) * inv, __uint_as_float(orr[v * 8 + 1]) * inv);
-                            o4.y = pack_bf16(__uint_as_float(orr[v * 8 + 2]) * inv, __uint_as_float(orr[v * 8 + 3]) * inv);
-                            o4.z = pack_bf16(__uint_as_float(orr[v * 8 + 4]) * inv, __uint_as_float(orr[v * 8 + 5]) * inv);
-                            o4.w = pack_bf16(__uint_as_float(orr[v * 8 + 6]) * inv, __uint_as_float(orr[v * 8 + 7]) * inv);
-                            *reinterpret_cast<uint4*>(orow + c * 32 + v * 8) = o4;
+                            uint32_t o8[8];
+#pragma unroll
+                            for (int j = 0; j < 8; ++j) {
+                                const int e = v * 16 + 2 * j;
+                                o8[j] = pack_bf16(__uint_as_float(orr[e >> 5][e & 31]) * inv, __uint_as_float(orr[e >> 5][(e & 31) + 1]) * inv);
+                            }
+                            stg_256(orow + c * 64 + v * 16, o8);
                         }
                     }
                 }
