@@ -16,13 +16,13 @@ constexpr int kPage = 16;             // tokens per KV page (BASELINE.json confi
 constexpr int kTileKeys = 128;        // keys per staged KV tile / MMA N
 constexpr int kTileRows = 128;        // query rows per prefill tile / MMA M
 constexpr int kMaxGroup = 16;         // max q heads per kv head on the decode path (MMA M = 16)
-constexpr int kDecodeWaves = 6;       // target decode items per SM when choosing the split length
+constexpr int kDecodeWaves = 3;       // target decode items per SM when choosing the split length
 constexpr int kMinSplitKeys = 512;    // never split a decode KV range finer than this
 constexpr int kMaxSplitKeys = 4096;   // never leave a decode item longer than this
 // SM partition model of the two-queue scheduler (measured on B200): bytes/us one SM streams on the
 // decode path, flop/us one SM sustains on the prefill path, and the CTA count past which decode is HBM-limited.
 constexpr float kDecodeBytesPerUsPerSm = 80e3f;
-constexpr float kPrefillFlopsPerUsPerSm = 6.0e6f;
+constexpr float kPrefillFlopsPerUsPerSm = 8.0e6f;
 constexpr int kMaxDecodeCtas = 88;
 // ss_debug_set_param keys (tuning / measurement aids; 0 restores the automatic choice)
 enum { kDbgGrid = 1, kDbgDecodeCtas = 2, kDbgSplitKeys = 3, kDbgTwoKernel = 4 };
