@@ -21,6 +21,7 @@ struct PlanHeader {                  // lives in shared memory
     int32_t nP, nD;                  // prefill / decode requests
     int32_t tot_p, tot_d;            // prefill / decode items
     int32_t n_decode_ctas;           // CTAs [0, n) drain the decode queue first
+    int32_t pair_heads;              // 1: a prefill item serves two query heads of a kv head (two softmax chains per CTA)
     unsigned long long total_keys;   // sum over D of (u + 1)
     unsigned long long total_pairs;  // sum over P of c*u + c(c+1)/2
 };
@@ -35,8 +36,13 @@ struct PlanTables {
 
 __device__ __forceinline__ int plan_ceil_div(int a, int b) { return (a + b - 1) / b; }
 
-// prefill items per (request, row tile): Hkv groups x ceil(G / 2) head pairs
+// prefill items per (request, row tile): Hkv groups x ceil(G / 2) head pairs, or one per query head
 __host__ __device__ __forceinline__ int plan_head_pairs(int Hq, int Hkv) { return Hkv * ((Hq / Hkv + 1) / 2); }
+// Pair two heads per item unless the single-head items would all fit in one wave of CTAs anyway: a pair item keeps a
+// CTA ~1.6x as long as a single-head item (two chains share the SM), so pairing pays only from the second wave on.
+__host__ __device__ __forceinline__ int plan_pair_heads(int row_tiles, int Hq, int Hkv, int prefill_ctas) {
+    return Hq / Hkv > 1 && row_tiles * Hq > prefill_ctas;
+}
 
 // balanced split of n keys into ceil(n / L) tile-aligned chunks
 __device__ __forceinline__ int plan_decode_chunk(int n, int L) {
@@ -152,13 +158,11 @@ __device__ void build_plan(const int32_t* __restrict__ qsl, const int32_t* __res
             carry += __shfl_sync(0xffffffffu, incl, 31);
         }
         if (lane == 0) {
-            const int tot_p = tiles_p * plan_head_pairs(Hq, Hkv), tot_d = carry * Hkv;
-            ph->tot_p = tot_p;
-            ph->tot_d = tot_d;
+            const int tot_d = carry * Hkv;
             // SM partition between the two queues: SM-time of the decode items at the per-SM streaming rate vs SM-time
             // of the prefill tiles at the per-SM tensor rate; never more decode-first CTAs than saturate HBM.
             int nd = 0;
-            if (tot_d > 0 && tot_p == 0) nd = num_sms;
+            if (tot_d > 0 && tiles_p == 0) nd = num_sms;
             else if (tot_d > 0) {
                 const float t_d = (float)ph->total_keys * (float)(Hkv * D * 4) / kDecodeBytesPerUsPerSm;
                 const float t_p = (float)ph->total_pairs * (float)Hq * (float)(4 * D) / kPrefillFlopsPerUsPerSm;
@@ -169,6 +173,11 @@ __device__ void build_plan(const int32_t* __restrict__ qsl, const int32_t* __res
             }
             if (force_decode_ctas > 0) nd = force_decode_ctas;
             if (force_decode_ctas < 0) nd = 0;
+            const int pair = plan_pair_heads(tiles_p, Hq, Hkv, num_sms - (nd < num_sms ? nd : 0));
+            ph->pair_heads = pair;
+            const int tot_p = tiles_p * (pair ? plan_head_pairs(Hq, Hkv) : Hq);
+            ph->tot_p = tot_p;
+            ph->tot_d = tot_d;
             ph->n_decode_ctas = nd;
         }
     }
@@ -182,7 +191,7 @@ __device__ __forceinline__ void plan_decode_item(int idx, const PlanHeader* ph, 
                                                  int Hq, int Hkv, ss_work_item& it) {
     const int nP = ph->nP;
     if (idx < ph->tot_p) {
-        const int G = Hq / Hkv, GP = (G + 1) / 2, HP = Hkv * GP;
+        const int G = Hq / Hkv, GP = ph->pair_heads ? (G + 1) / 2 : G, HP = Hkv * GP, hpi = ph->pair_heads ? 2 : 1;
         const int unit = idx / HP;
         int lo = 0, hi = nP;                             // last k with off[k] <= unit
         while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if ((int)tb.off[mid] <= unit) lo = mid; else hi = mid; }
@@ -192,9 +201,9 @@ __device__ __forceinline__ void plan_decode_item(int idx, const PlanHeader* ph, 
         const int mt = ntile - 1 - local / HP;           // heaviest (last) tile first
         const int nrows = min(kTileRows, c - mt * kTileRows);
         const int hp = local % HP, g = hp / GP, j = hp % GP;
-        it.kind = 1; it.req = r; it.head = g * G + 2 * j; it.row0 = q0 + mt * kTileRows; it.nrows = nrows;
+        it.kind = 1; it.req = r; it.head = g * G + hpi * j; it.row0 = q0 + mt * kTileRows; it.nrows = nrows;
         it.kv_begin = 0; it.kv_end = u + mt * kTileRows + nrows; it.split = 0; it.nsplit = 1;
-        it.partial = -1; it.q_pos0 = mt * kTileRows; it.nheads = (2 * j + 1 < G) ? 2 : 1;
+        it.partial = -1; it.q_pos0 = mt * kTileRows; it.nheads = (hpi == 2 && 2 * j + 1 < G) ? 2 : 1;
     } else {
         const int didx = idx - ph->tot_p, unit = didx / Hkv;
         int lo = 0, hi = ph->nD;
