@@ -100,6 +100,20 @@ int ss_kv_append(ss_handle* h, const void* k_new, const void* v_new, const int32
                  void* cuda_stream);
 
 /*
+ * The step before the path: RoPE + QKV split fused into the append.  qkv is the fused
+ * projection output [T][(Hq + 2 Hkv) * D] bf16 - per token the Hq query heads, then the Hkv key heads, then the Hkv value
+ * heads.  q and k are rotated by the token's absolute position ctx_lens[r] + j with the "rotate-half" rotary embedding
+ * of the model families the paper serves (reading 22):
+ *     angle_i = pos * rope_theta^(-2i/D);  y_i = x_i cos - x_{i+D/2} sin;  y_{i+D/2} = x_{i+D/2} cos + x_i sin
+ * (cos / sin evaluated in double, the rotation in fp32, one rounding to bf16).  Rotated q -> q_out [T][Hq][D] (the q
+ * argument of ss_mixed_attention), rotated k and the untouched v bits -> their page slots exactly as ss_kv_append places
+ * them.  Replaces ss_kv_append for the batch.  rope_theta must be finite and > 1.  All pointers device.
+ */
+int ss_qkv_rope_append(ss_handle* h, const void* qkv, const int32_t* block_table, const int32_t* query_start_loc,
+                       const int32_t* ctx_lens, int32_t R, int32_t T, float rope_theta, void* q_out,
+                       void* cuda_stream);
+
+/*
  * a2..a5  mixed_attention (north_star "mixed_attention(q, k_cache, v_cache,
  * block_table, query_start_loc, ctx_lens, scale, out)"; the caches were bound at ss_create).
  * For request r, row j < c_r, head h:  out = softmax(scale * q . K[0..u_r+j]^T) V[0..u_r+j]  with

@@ -20,7 +20,7 @@ SS_ERR_DEVICE_CHECK = -6
 SS_FLAG_DEBUG_CHECKS = 1
 # include/slidingattn.h (the product boundary) ...
 EXPORTS = ["ss_version", "ss_status_string", "ss_last_error_string", "ss_create", "ss_destroy",
-           "ss_workspace_bytes", "ss_kv_append", "ss_mixed_attention", "ss_iteration_host",
+           "ss_workspace_bytes", "ss_kv_append", "ss_qkv_rope_append", "ss_mixed_attention", "ss_iteration_host",
            "ss_poll_device_error", "ss_reset"]
 # ... and include/slidingattn_debug.h (test / tuning / measurement aids)
 DEBUG_EXPORTS = ["ss_build_worklist", "ss_last_launch_count", "ss_debug_force_simple_path",
@@ -68,6 +68,7 @@ def load():
     lib.ss_workspace_bytes.argtypes = [vp]
     lib.ss_workspace_bytes.restype = ctypes.c_size_t
     lib.ss_kv_append.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, vp]
+    lib.ss_qkv_rope_append.argtypes = [vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
     lib.ss_mixed_attention.argtypes = [vp, vp, vp, vp, vp, i32, i32, f32, vp, vp, vp, ctypes.c_size_t, vp]
     lib.ss_build_worklist.argtypes = [vp, vp, vp, i32, i32, vp, ctypes.c_size_t, vp, i32,
                                       ctypes.POINTER(i32 * 3), vp]
@@ -166,6 +167,19 @@ class SlidingAttn:
         _want(v_new, "v_new", torch.bfloat16, True, kv_shape)
         self._check(self.lib.ss_kv_append(self._h, _ptr(k_new), _ptr(v_new), _ptr(block_table),
                                           _ptr(query_start_loc), _ptr(ctx_lens), R, T, _stream_ptr(stream)))
+
+    def qkv_rope_append(self, qkv, block_table, query_start_loc, ctx_lens, rope_theta, q_out=None, stream=None):
+        """RoPE + QKV split fused into the append (NEXT-4): returns the rotated q [T, Hq, D]."""
+        R, T = self._check_batch(block_table, query_start_loc, ctx_lens), qkv.shape[0]
+        c = self.cfg
+        _want(qkv, "qkv", torch.bfloat16, True, (T, (c.num_q_heads + 2 * c.num_kv_heads) * c.head_dim))
+        if q_out is None:
+            q_out = torch.empty(T, c.num_q_heads, c.head_dim, dtype=torch.bfloat16, device=qkv.device)
+        _want(q_out, "q_out", torch.bfloat16, True, (T, c.num_q_heads, c.head_dim))
+        self._check(self.lib.ss_qkv_rope_append(self._h, _ptr(qkv), _ptr(block_table), _ptr(query_start_loc),
+                                                _ptr(ctx_lens), R, T, float(rope_theta), _ptr(q_out),
+                                                _stream_ptr(stream)))
+        return q_out
 
     def mixed_attention(self, q, block_table, query_start_loc, ctx_lens, scale, out=None, lse=None,
                         stream=None):

@@ -243,6 +243,23 @@ int ss_kv_append(ss_handle* hh, const void* k_new, const void* v_new, const int3
     return SS_OK;
 }
 
+int ss_qkv_rope_append(ss_handle* hh, const void* qkv, const int32_t* block_table, const int32_t* query_start_loc,
+                       const int32_t* ctx_lens, int32_t R, int32_t T, float rope_theta, void* q_out, void* cuda_stream) {
+    Handle* h = (Handle*)hh;
+    int rc = check_batch_args(h, qkv, q_out, query_start_loc, ctx_lens, R, T);
+    if (rc != SS_OK) return rc;
+    h->last_launches = 0;
+    if (R == 0 || T == 0) return SS_OK;
+    if (!block_table || (((uintptr_t)block_table) & 3u)) return SS_ERR_INVALID_ARG;
+    if (!(rope_theta > 1.f) || !isfinite(rope_theta)) return SS_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (h->debug_checks) SS_CUDA(h, launch_validate(h, block_table, query_start_loc, ctx_lens, R, T, st), "validate launch");
+    SS_CUDA(h, launch_qkv_rope_append(h, qkv, block_table, query_start_loc, ctx_lens, R, T, rope_theta, q_out, st),
+            "qkv_rope_append launch");
+    h->last_launches = 1 + h->debug_checks;
+    return SS_OK;
+}
+
 int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table, const int32_t* query_start_loc,
                        const int32_t* ctx_lens, int32_t R, int32_t T, float scale, void* out, float* lse_or_null,
                        void* workspace, size_t workspace_bytes, void* cuda_stream) {

@@ -122,6 +122,8 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
 // ---- launchers implemented in the .cu files (all enqueue on `stream`, return cudaError_t) ----
 cudaError_t launch_kv_append(const Handle* h, const void* k_new, const void* v_new, const int32_t* bt,
                              const int32_t* qsl, const int32_t* ctx, int R, int T, cudaStream_t stream);
+cudaError_t launch_qkv_rope_append(const Handle* h, const void* qkv, const int32_t* bt, const int32_t* qsl,
+                                   const int32_t* ctx, int R, int T, float rope_theta, void* q_out, cudaStream_t stream);
 cudaError_t launch_worklist(const Handle* h, const int32_t* qsl, const int32_t* ctx, int R, int T,
                             void* workspace, cudaStream_t stream);
 cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_t* bt, const int32_t* qsl,
