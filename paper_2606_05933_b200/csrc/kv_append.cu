@@ -2,12 +2,13 @@
 // One CTA per (token, K|V): the token's Hkv*D bf16 row is moved as 16-byte vectors straight into its
 // page slot.  Integer index math + bit copies only (never through a float type) => bit-exact.
 // Roofline: HBM; algorithmic bytes = 4*T*Hkv*D*2 (read + write, K and V).
+#include "append.cuh"
 #include "common.cuh"
 #include "ptx.cuh"
 
 namespace ss {
 
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(kAppendThreads)
 kv_append_kernel(const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
                  uint4* __restrict__ k_cache, uint4* __restrict__ v_cache,
                  const int32_t* __restrict__ block_table, const int32_t* __restrict__ qsl,
@@ -20,24 +21,22 @@ kv_append_kernel(const uint4* __restrict__ k_new, const uint4* __restrict__ v_ne
     const uint4* __restrict__ src = blockIdx.y ? v_new : k_new;
     uint4* __restrict__ dst = blockIdx.y ? v_cache : k_cache;
 
-    // request of this token: last r with qsl[r] <= tok (empty requests are skipped by construction)
-    int lo = 0, hi = R;            // invariant: qsl[lo] <= tok < qsl[hi]
-    while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (__ldg(qsl + mid) <= tok) lo = mid; else hi = mid;
-    }
-    const int r = lo;
+    // the token's first vectors are requested before the (dependent) metadata chain, so the two overlap
+    const int vec_per_tok = Hkv * vec_per_head;
+    const uint4* s = src + (int64_t)tok * vec_per_tok;
+    uint4 first = make_uint4(0u, 0u, 0u, 0u);
+    if ((int)threadIdx.x < vec_per_tok) first = __ldg(s + threadIdx.x);
+
+    const int r = request_of_token(qsl, R, tok);
     const int pos = __ldg(ctx_lens + r) + (tok - __ldg(qsl + r));
     const int64_t page = __ldg(block_table + (int64_t)r * max_pages + (pos >> 4));
     const int slot = pos & (kPage - 1);
 
-    const int vec_per_tok = Hkv * vec_per_head;
-    const uint4* s = src + (int64_t)tok * vec_per_tok;
-    for (int v = threadIdx.x; v < vec_per_tok; v += blockDim.x) {
+    for (int v = threadIdx.x; v < vec_per_tok; v += kAppendThreads) {
         const int g = v / vec_per_head;
         const int dv = v - g * vec_per_head;
         const int64_t d = ((page * Hkv + g) * kPage + slot) * (int64_t)vec_per_head + dv;
-        dst[d] = __ldg(s + v);
+        dst[d] = v == (int)threadIdx.x ? first : __ldg(s + v);
     }
 }
 
@@ -45,7 +44,7 @@ cudaError_t launch_kv_append(const Handle* h, const void* k_new, const void* v_n
                              const int32_t* qsl, const int32_t* ctx, int R, int T, cudaStream_t stream) {
     const ss_config& c = h->cfg;
     dim3 grid((unsigned)T, 2, 1);
-    return launch_pdl(kv_append_kernel, grid, dim3(128), 0, stream, (const uint4*)k_new, (const uint4*)v_new,
+    return launch_pdl(kv_append_kernel, grid, dim3(kAppendThreads), 0, stream, (const uint4*)k_new, (const uint4*)v_new,
                       (uint4*)h->k_cache, (uint4*)h->v_cache, bt, qsl, ctx, R, c.max_pages_per_req, c.num_kv_heads,
                       c.head_dim / 8, (const int32_t*)(h->debug_checks ? h->state + kStateErr : nullptr));
 }

@@ -7,12 +7,13 @@
 // (the a1 write).  One CTA per token: cos / sin of the D/2 angles are evaluated ONCE per token in double (range reduction
 // at positions up to 2^30 needs it; 64 values, negligible) and shared through smem by all Hq + Hkv heads; the rotation
 // itself is fp32 on bf16 pairs, one rounding to bf16.  HBM-bound: reads (Hq + 2 Hkv) D 2 bytes per token, writes the same.
+#include "append.cuh"
 #include "common.cuh"
 #include "ptx.cuh"
 
 namespace ss {
 
-constexpr int kRopeThreads = 128;
+constexpr int kRopeThreads = kAppendThreads;
 
 __device__ __forceinline__ float2 bf2_to_f2(uint32_t w) {
     return make_float2(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u));
@@ -28,12 +29,7 @@ qkv_rope_append_kernel(const uint32_t* __restrict__ qkv, uint32_t* __restrict__ 
     ptx::pdl_wait();
     if (err_flag && *reinterpret_cast<const volatile int32_t*>(err_flag)) return;    // debug checks tripped: write nothing
     const int tok = blockIdx.x, tid = threadIdx.x;
-    int lo = 0, hi = R;            // last r with qsl[r] <= tok
-    while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (__ldg(qsl + mid) <= tok) lo = mid; else hi = mid;
-    }
-    const int r = lo;
+    const int r = request_of_token(qsl, R, tok);
     const int pos = __ldg(ctx_lens + r) + (tok - __ldg(qsl + r));
     const int64_t page = __ldg(block_table + (int64_t)r * max_pages + (pos >> 4));
     const int slot = pos & (kPage - 1);
