@@ -39,8 +39,12 @@ int fail_cuda(Handle* h, cudaError_t e, const char* where) {
         if (e__ != cudaSuccess) return fail_cuda(h, e__, where); \
     } while (0)
 
-// KV cache viewed as a 2-D bf16 matrix [num_pages*Hkv*16 rows][D]; one TMA box = one page slab half:
-// 16 rows x 64 columns (128 bytes, SWIZZLE_128B), the canonical K-major UMMA / ldmatrix atom.
+// KV cache [num_pages][Hkv][16][D] bf16 viewed as a 4-D tensor (innermost first): 64 columns of a 128-byte half row,
+// 8 rows of an 8-key group (stride D*2 bytes), D/64 halves (stride 128 bytes), 8-key groups (stride 8*D*2 bytes; a
+// (page, kv head) slab is two consecutive groups).  One TMA box = one whole slab: 2 groups x halves x 8 rows x 64
+// columns, written to shared memory as [group][half][8 rows][128 B] with SWIZZLE_128B - every [8 rows][128 B] block is a
+// canonical UMMA / ldmatrix core group, groups uniformly D/64 KB apart.  One operation per slab instead of one per
+// (slab, half): the per-SM copy engine costs ~31 ns per operation whatever its size (profiles/r2b.md).
 int encode_cache_map(Handle* h, CUtensorMap* map, void* base) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) {
@@ -48,11 +52,12 @@ int encode_cache_map(Handle* h, CUtensorMap* map, void* base) {
         return SS_ERR_CUDA;
     }
     const ss_config& c = h->cfg;
-    cuuint64_t gdim[2] = {(cuuint64_t)c.head_dim, (cuuint64_t)c.num_pages * c.num_kv_heads * kPage};
-    cuuint64_t gstride[1] = {(cuuint64_t)c.head_dim * 2};
-    cuuint32_t box[2] = {64u, (cuuint32_t)kPage};
-    cuuint32_t estr[2] = {1u, 1u};
-    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, base, gdim, gstride, box, estr,
+    const cuuint32_t halves = (cuuint32_t)c.head_dim / 64;
+    cuuint64_t gdim[4] = {64, 8, halves, (cuuint64_t)c.num_pages * c.num_kv_heads * 2};
+    cuuint64_t gstride[3] = {(cuuint64_t)c.head_dim * 2, 128, (cuuint64_t)c.head_dim * 2 * 8};
+    cuuint32_t box[4] = {64u, 8u, halves, 2u};
+    cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, base, gdim, gstride, box, estr,
                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {

@@ -5,11 +5,13 @@
 // counter), so tensor-bound prefill tiles and HBM-bound decode splits overlap across SMs and the batch
 // costs ~max(bytes/HBM, flops/tensor) instead of the sum.  12 warps per CTA in 3 warpgroups; the register
 // file is re-partitioned with setmaxnreg (WG0 72 registers per thread, WG1 / WG2 216):
-//   WG0 warp 0  scheduler + TMA producer (one elected thread).  Publishes each item to the other warps through a
+//   WG0 warp 0  scheduler + Q / K producer (one elected thread).  Publishes each item to the other warps through a
 //               4-slot smem ring, loads the Q tiles (prefill: the item's 1 or 2 query heads, 128 rows each) and
-//               streams 64-key K and V tiles — 4 pages x D/64 boxes of 16 rows x 128 B, SWIZZLE_128B — into
-//               separate 5-slot K and V rings (a K slot is free as soon as its S MMAs are done, a V slot as soon
-//               as its PV MMAs are done).
+//               streams 64-key K tiles into a 5-slot K ring: ONE 4-D TMA box per (page, kv head) slab (16 keys x D,
+//               SWIZZLE_128B, written as [8-key group][64-column half][8 rows][128 B]).
+//   WG0 warp 3  V producer (one elected thread): follows the item ring and streams the V tiles the same way into the
+//               V ring (a K slot is free as soon as its S MMAs are done, a V slot as soon as its PV MMAs are done).
+//               Two producer threads because one could not issue a 32 KB tile in less than ~600 ns.
 //   WG0 warps 1,2  tcgen05.mma issuers (warp 1 also owns the TMEM allocation), one elected thread each: warp 1 issues
 //               chain A's MMAs, warp 2 chain B's (prefill items only).  Per query head X (a
 //               "chain") TMEM holds S_X[0], S_X[1] (128 rows x 64 keys fp32, 64 columns each) and O_X (128 x D
@@ -17,17 +19,18 @@
 //               chain the order is  S(k) -> softmax -> P(k) -> PV(k) -> S(k+2)  with S(k+1) already done: each
 //               chain's softmax never waits for the tensor pipe, and the two chains interleave on it
 //               (PV_A(k) S_A(k+2) PV_B(k) S_B(k+2) ...) while sharing every staged K/V tile.
+//               Decode items: warp 2 runs a5 - publishes each split (acq_rel ticket) and, when it draws the last
+//               ticket of a (request, kv head), merges all splits in fixed order (bitwise reproducible).
 //   WG1, WG2    workers (4 warps each; warp % 4 = TMEM lane quarter).
 //               prefill item: WG1 = chain A (head), WG2 = chain B (head + 1); thread = query row (TMEM lane):
 //                 tcgen05.ld S, causal/length mask by select (only in the warp-uniform diagonal variant), online
 //                 softmax (exp2, log2e folded into the scale, packed f32x2 arithmetic, lazy rescale: O is only touched
 //                 when a row max grows by more than 2^8), P -> bf16 -> TMEM, epilogue stores rows < nrows only.
-//               decode item: WG1 warp w owns 32 keys of a pair of 64-key slots: mma.sync.m16n8k16 with the G query
-//                 heads of the KV head padded to 16 rows (bandwidth-bound, wasted rows are free), online softmax
-//                 in registers with quad shuffles, cross-warp log-sum-exp merge through smem, then either the
-//                 final bf16 row or an fp32 partial.  WG2 warp 0 runs a5 meanwhile: it publishes each split
-//                 (acq_rel ticket) and, when it draws the last ticket of a (request, kv head), merges all splits
-//                 in fixed order (bitwise reproducible).
+//               decode item: all 8 worker warps; a warp owns 16 keys of every other 64-key slot (WG1 the even slots
+//                 of the item, WG2 the odd ones): mma.sync.m16n8k16 with the G query heads of the KV head padded to 16
+//                 rows (bandwidth-bound, wasted rows are free), online softmax in registers with quad shuffles,
+//                 two-stage cross-warp log-sum-exp merge through smem (WG2 -> WG1 in registers, then 4 -> 1), then
+//                 either the final bf16 row or an fp32 partial.
 // Rooflines: decode items HBM (2*D*2 bytes per cached token per kv head), prefill items bf16 tensor
 // (4*D flop per visible (row,key) pair per head).  V rows at/after kv_end are zeroed in smem before any
 // PV product (unused slots may hold NaN; 0*NaN = NaN); masked scores are replaced, never multiplied.
@@ -52,8 +55,12 @@ using namespace ptx;
 
 constexpr int kMixThreads = 384;
 constexpr int kSlotKeys = 64;        // keys per K / V ring slot = keys per S buffer
-constexpr int kNumSt = 5;            // K ring slots = V ring slots
+#ifndef SS_NUM_ST
+#define SS_NUM_ST 5
+#endif
+constexpr int kNumSt = SS_NUM_ST;    // K ring slots = V ring slots
 constexpr int kSchedSlots = 4;
+constexpr int kDecKeys = 16;         // keys of a 64-key slot one decode warp owns (4 warps per slot)
 // setmaxnreg moves registers inside the CTA's own launch allocation: 384 threads x 168 (the __launch_bounds__ cap ptxas
 // reports) = 64512, so 128*72 + 256*216 = 64512 fits exactly; one register more per worker and the .inc spins forever.
 constexpr int kRegsLaunch = 168, kRegsWg0 = 72, kRegsWorker = 216;
@@ -66,11 +73,26 @@ template <int D>
 struct MixSmem {
     static constexpr int kHalves = D / 64;
     static constexpr int kSlot = kHalves * kSlotKeys * 128;      // one K (or V) ring slot
+    // Slot layout = what ONE 4-D TMA box per (page, kv head) slab writes: [8-key group][64-column half][8 rows][128 B],
+    // every [8 rows][128 B] block a SWIZZLE_128B core group.  8-key groups are kGroup bytes apart (uniform over the 4
+    // pages of a slot: the UMMA stride-byte-offset), the halves of a group 1024 bytes apart.
+    static constexpr int kGroup = kHalves * 1024;
+    static constexpr int kPageBytes = 2 * kGroup;                // one (page, kv head) slab: 16 keys
+    // byte offset of the 16-byte chunk cd (0 .. D/8-1) of key row r (0 .. 63) inside a slot, swizzle applied
+    __device__ static __forceinline__ uint32_t kv_off(int r, int cd) {
+        return (uint32_t)((r >> 3) * kGroup + (cd >> 3) * 1024 + (r & 7) * 128 + (((cd & 7) ^ (r & 7)) << 4));
+    }
     static constexpr int kQTile = kHalves * kTileRows * 128;     // one Q tile (one query head, 128 rows)
     static constexpr int kKOff = 0;
     static constexpr int kVOff = kKOff + kNumSt * kSlot;
     static constexpr int kQOff = kVOff + kNumSt * kSlot;         // 2 Q tiles (prefill) / decode: cross-warp merge buffer + staged Q rows
-    static constexpr int kQBytes = 2 * kQTile;
+#ifndef SS_Q_TILES
+#define SS_Q_TILES 2
+#endif
+#ifndef SS_Q_EXTRA
+#define SS_Q_EXTRA 0
+#endif
+    static constexpr int kQBytes = SS_Q_TILES * kQTile + SS_Q_EXTRA;
     static constexpr int kMergeBytes = 4 * kMaxGroup * (D + 2) * 4;
     // decode with G <= 8: merge buffer of 8 rows per warp, then kSchedSlots staged Q blocks (G rows x D bf16, one per
     // scheduler slot, bulk-copied by the producer so the workers never wait on a cold global Q load)
@@ -94,13 +116,14 @@ struct MixSmem {
 
 // barrier indices (8 bytes each, from kBarOff)
 enum : int {
-    B_KFULL = 0, B_VFULL = 5, B_KEMPTY_P = 10, B_KEMPTY_D = 15, B_VEMPTY_P = 20, B_VEMPTY_D = 25,
-    B_SFULL = 30, B_PFULL = 34,                       // [chain * 2 + buffer]
-    B_QFULL = 38, B_QEMPTY = 39, B_OFULL = 40, B_OFREE = 42, B_PVDONE = 44,     // [chain]
-    B_SCHED_FULL = 46, B_SCHED_EMPTY = 50, B_PARTIAL = 54, B_COUNT = 58
+    B_KFULL = 0, B_VFULL = kNumSt, B_KEMPTY_P = 2 * kNumSt, B_KEMPTY_D = 3 * kNumSt, B_VEMPTY_P = 4 * kNumSt,
+    B_VEMPTY_D = 5 * kNumSt,
+    B_SFULL = 6 * kNumSt, B_PFULL = B_SFULL + 4,      // [chain * 2 + buffer]
+    B_QFULL = B_PFULL + 4, B_QEMPTY = B_QFULL + 1, B_OFULL = B_QEMPTY + 1, B_OFREE = B_OFULL + 2, B_PVDONE = B_OFREE + 2,     // [chain]
+    B_SCHED_FULL = B_PVDONE + 2, B_SCHED_EMPTY = B_SCHED_FULL + 4, B_PARTIAL = B_SCHED_EMPTY + 4, B_COUNT = B_PARTIAL + 4
 };
 static_assert(B_COUNT * 8 <= 512, "barrier region");
-static_assert(kNumSt == 5, "barrier indices assume 5 ring slots");
+static_assert(kSchedSlots == 4, "barrier indices assume 4 scheduler slots");
 
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
     uint64_t d = 0;
@@ -191,6 +214,308 @@ __device__ __forceinline__ float softmax_half(uint32_t (&sr)[2][32], int nvis, f
     return alpha;
 }
 
+// One decode split on the 8 worker warps (see the call site).  NT = 8-head column tiles (1: G <= 8, 2: G <= 16).
+template <int D, int NT>
+__device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, const int slot, const uint32_t tile_ctr,
+                                            const int wg, const int cw, const int lane, const int wtid, const uint32_t sbase,
+                                            const uint32_t bar0, const MixParams& prm, float* merge, unsigned long long* tr) {
+    using SM = MixSmem<D>;
+    constexpr int kHalves = SM::kHalves;
+    auto BAR = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
+    const int Hq = prm.Hq, Hkv = prm.Hkv, G = Hq / Hkv;
+    const float sl2 = prm.scale * kMLog2e;
+    const int qr = lane >> 2, qc = (lane & 3) * 2;           // fragment coordinates: row / column pair
+    constexpr int mrows = NT * 8;                           // merge-buffer rows (heads) per warp
+    // B fragments of Q^T (16 d x 8 heads per k-step): head = 8 nt + qr, d = 16 ks + qc (+1) and + 8
+    uint32_t qb[D / 16][2 * NT];
+    if (NT == 1) {
+        const uint32_t qs = sbase + SM::kQStageOff + slot * SM::kQStageBytes + (qr * D + qc) * 2;
+#pragma unroll
+        for (int ks = 0; ks < D / 16; ++ks) {
+            qb[ks][0] = qr < G ? lds32(qs + ks * 32) : 0u;
+            qb[ks][1] = qr < G ? lds32(qs + ks * 32 + 16) : 0u;
+        }
+    } else {
+        const __nv_bfloat16* qg = prm.q + ((int64_t)w.row0 * Hq + (int64_t)w.head * G) * D;
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+            for (int ks = 0; ks < D / 16; ++ks) {
+                const int hd = 8 * nt + qr;
+                qb[ks][2 * nt] = hd < G ? *reinterpret_cast<const uint32_t*>(qg + (int64_t)hd * D + ks * 16 + qc) : 0u;
+                qb[ks][2 * nt + 1] = hd < G ? *reinterpret_cast<const uint32_t*>(qg + (int64_t)hd * D + ks * 16 + qc + 8) : 0u;
+            }
+    }
+    // O^T accumulators: [nt][mt] c0 = (d = 16 mt + qr, head 8 nt + qc), c1 = head + 1, c2 = (d + 8, head), c3 = (d + 8, head + 1)
+    float oT[NT][D / 16][4];
+    float m[NT][2], l[NT][2];                               // per head qc, qc + 1 (l: this lane's share of the row sum)
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        m[nt][0] = m[nt][1] = -INFINITY;
+        l[nt][0] = l[nt][1] = 0.f;
+#pragma unroll
+        for (int mt = 0; mt < D / 16; ++mt) oT[nt][mt][0] = oT[nt][mt][1] = oT[nt][mt][2] = oT[nt][mt][3] = 0.f;
+    }
+    // EVERY warp waits FULL and arrives EMPTY on EVERY slot: an mbarrier parity wait is only sound while the waiter is less
+    // than one phase away from the barrier, and with 5 ring slots a slot alternates between the two warpgroups.
+    const int r16 = cw * kDecKeys;                          // first key row of this warp inside its slots
+    const int mi = lane >> 3, l7 = lane & 7;                // ldmatrix: this lane addresses row l7 of matrix mi
+    for (int t = 0; t < n; ++t) {
+        const uint32_t tc = tile_ctr + t;
+        const int s = tc % kNumSt;
+        const uint32_t fpar = (tc / kNumSt) & 1;
+        const int key0 = w.kv_begin + t * kSlotKeys;
+        const int nvalid = (t & 1) == wg ? w.kv_end - (key0 + r16) : 0;       // <= 0: nothing for this warp in this slot
+        const uint32_t kbase = sbase + SM::kKOff + s * SM::kSlot;
+        const uint32_t vbase = sbase + SM::kVOff + s * SM::kSlot;
+        float sT[NT][4];
+        mbar_wait(BAR(B_KFULL + s), fpar);
+        if (tr && t == 0) tr[3] = globaltimer_ns();
+        if (nvalid > 0) {
+            // S^T (16 keys x 8 heads) = K (16 x D) Q^T: two interleaved accumulation chains per head tile
+            float sU[NT][4];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) sT[nt][i] = sU[nt][i] = 0.f;
+            const int rk = r16 + (mi & 1) * 8 + l7;          // a0: keys 0-7, a1: keys 8-15, a2 / a3: the next 8 d
+#pragma unroll
+            for (int ks = 0; ks < D / 16; ++ks) {
+                const int cd = 2 * ks + (mi >> 1);
+                uint32_t a[4];
+                ldmatrix_x4(a[0], a[1], a[2], a[3], kbase + SM::kv_off(rk, cd));
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) mma_bf16_16816((ks & 1) ? sU[nt] : sT[nt], a, qb[ks][2 * nt], qb[ks][2 * nt + 1]);
+            }
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                for (int i = 0; i < 4; ++i) sT[nt][i] += sU[nt][i];
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(BAR(B_KEMPTY_D + s));
+        mbar_wait(BAR(B_VFULL + s), fpar);
+        if (nvalid > 0) {
+            if (nvalid < kDecKeys) {
+                // zero the V rows past the end of the KV range (unused slots may hold NaN; 0 * NaN = NaN)
+                for (int i = lane; i < (kDecKeys - nvalid) * kHalves * 8; i += 32) {
+                    const int r = r16 + nvalid + i / (kHalves * 8);
+                    const int c = i % (kHalves * 8);
+                    const uint32_t a = vbase + SM::kv_off(r, c);
+                    asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
+                }
+                __syncwarp();
+            }
+            uint32_t pb[NT][2];                              // B fragments of P^T (16 keys x 8 heads)
+            bool moved = false;
+            float mn[NT][2];
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) {
+                // c0 / c1: key qr, heads qc / qc + 1;  c2 / c3: key qr + 8.  Masked by select, never by arithmetic.
+                if (qr >= nvalid) { sT[nt][0] = -INFINITY; sT[nt][1] = -INFINITY; }
+                if (qr + 8 >= nvalid) { sT[nt][2] = -INFINITY; sT[nt][3] = -INFINITY; }
+                float b0 = fmaxf(sT[nt][0], sT[nt][2]), b1 = fmaxf(sT[nt][1], sT[nt][3]);
+#pragma unroll
+                for (int o = 4; o < 32; o <<= 1) {
+                    b0 = fmaxf(b0, __shfl_xor_sync(0xffffffffu, b0, o));
+                    b1 = fmaxf(b1, __shfl_xor_sync(0xffffffffu, b1, o));
+                }
+                mn[nt][0] = fmaxf(m[nt][0], b0 * sl2);
+                mn[nt][1] = fmaxf(m[nt][1], b1 * sl2);
+                moved |= mn[nt][0] != m[nt][0] || mn[nt][1] != m[nt][1];
+                const float p0 = exp2f(sT[nt][0] * sl2 - mn[nt][0]), p1 = exp2f(sT[nt][1] * sl2 - mn[nt][1]);
+                const float p2 = exp2f(sT[nt][2] * sl2 - mn[nt][0]), p3 = exp2f(sT[nt][3] * sl2 - mn[nt][1]);
+                sT[nt][0] = p0 + p2;                         // this lane's share of the two row sums
+                sT[nt][1] = p1 + p3;
+                pb[nt][0] = movmatrix_trans(pack_bf16(p0, p1));   // keys 0-7:  (key qr, heads qc..) -> (head qr, keys qc..)
+                pb[nt][1] = movmatrix_trans(pack_bf16(p2, p3));   // keys 8-15
+            }
+            // the accumulators are only rescaled when some head's maximum moved (warp-uniform test)
+            if (__any_sync(0xffffffffu, moved)) {
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const float al0 = exp2f(m[nt][0] - mn[nt][0]), al1 = exp2f(m[nt][1] - mn[nt][1]);   // first tile: exp2(-inf) = 0
+                    l[nt][0] *= al0;
+                    l[nt][1] *= al1;
+#pragma unroll
+                    for (int mt = 0; mt < D / 16; ++mt) { oT[nt][mt][0] *= al0; oT[nt][mt][1] *= al1; oT[nt][mt][2] *= al0; oT[nt][mt][3] *= al1; }
+                    m[nt][0] = mn[nt][0];
+                    m[nt][1] = mn[nt][1];
+                }
+            }
+#pragma unroll
+            for (int nt = 0; nt < NT; ++nt) { l[nt][0] += sT[nt][0]; l[nt][1] += sT[nt][1]; }
+            // O^T (D x 8 heads) += V^T (D x 16 keys) P^T: a0 = (keys 0-7, d 0-7)^T, a1 = (keys 0-7, d 8-15)^T, a2 / a3: keys 8-15
+            const int rv = r16 + (mi >> 1) * 8 + l7;
+#pragma unroll
+            for (int mt = 0; mt < D / 16; ++mt) {
+                const int cd = 2 * mt + (mi & 1);
+                uint32_t a[4];
+                ldmatrix_x4_trans(a[0], a[1], a[2], a[3], vbase + SM::kv_off(rv, cd));
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) mma_bf16_16816(oT[nt][mt], a, pb[nt][0], pb[nt][1]);
+            }
+            if (nvalid < kDecKeys) fence_proxy_async();
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(BAR(B_VEMPTY_D + s));
+    }
+    // ---- cross-warp log-sum-exp merge through smem, two stages over one 4-warp buffer [warp][head][D + 2] ----
+    if (tr) tr[4] = globaltimer_ns();
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+            l[nt][0] += __shfl_xor_sync(0xffffffffu, l[nt][0], o);
+            l[nt][1] += __shfl_xor_sync(0xffffffffu, l[nt][1], o);
+        }
+    float* mine = merge + cw * mrows * (D + 2);
+    auto put = [&]() {
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) {
+            float* h0 = mine + (8 * nt + qc) * (D + 2);
+            float* h1 = h0 + (D + 2);
+#pragma unroll
+            for (int mt = 0; mt < D / 16; ++mt) {
+                h0[16 * mt + qr] = oT[nt][mt][0];
+                h1[16 * mt + qr] = oT[nt][mt][1];
+                h0[16 * mt + qr + 8] = oT[nt][mt][2];
+                h1[16 * mt + qr + 8] = oT[nt][mt][3];
+            }
+            if (qr == 0) {
+                h0[D] = m[nt][0]; h0[D + 1] = l[nt][0];
+                h1[D] = m[nt][1]; h1[D + 1] = l[nt][1];
+            }
+        }
+    };
+    if (wg == 1) {
+        // stage A: WG2's warp cw hands its partial to WG1's warp cw (same fragment coordinates).  The buffer is free
+        // once WG1 has finished the previous decode item's merge (named barrier 3: WG1 arrives, WG2 syncs).
+        named_bar_sync(3, 256);
+        put();
+        named_bar_arrive(2, 256);
+        return;
+    }
+    named_bar_sync(2, 256);
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+        const float* h0 = mine + (8 * nt + qc) * (D + 2);
+        const float* h1 = h0 + (D + 2);
+        const float mb0 = h0[D], lb0 = h0[D + 1], mb1 = h1[D], lb1 = h1[D + 1];
+        const float M0 = fmaxf(m[nt][0], mb0), M1 = fmaxf(m[nt][1], mb1);
+        // a side that saw no key has m = -inf: weight 0 (and never exp2(-inf - -inf))
+        const float wa0 = m[nt][0] == -INFINITY ? 0.f : exp2f(m[nt][0] - M0), wb0 = mb0 == -INFINITY ? 0.f : exp2f(mb0 - M0);
+        const float wa1 = m[nt][1] == -INFINITY ? 0.f : exp2f(m[nt][1] - M1), wb1 = mb1 == -INFINITY ? 0.f : exp2f(mb1 - M1);
+#pragma unroll
+        for (int mt = 0; mt < D / 16; ++mt) {
+            oT[nt][mt][0] = oT[nt][mt][0] * wa0 + h0[16 * mt + qr] * wb0;
+            oT[nt][mt][1] = oT[nt][mt][1] * wa1 + h1[16 * mt + qr] * wb1;
+            oT[nt][mt][2] = oT[nt][mt][2] * wa0 + h0[16 * mt + qr + 8] * wb0;
+            oT[nt][mt][3] = oT[nt][mt][3] * wa1 + h1[16 * mt + qr + 8] * wb1;
+        }
+        l[nt][0] = l[nt][0] * wa0 + lb0 * wb0;
+        l[nt][1] = l[nt][1] * wa1 + lb1 * wb1;
+        m[nt][0] = M0;
+        m[nt][1] = M1;
+    }
+    __syncwarp();                                 // this warp's reads of `mine` are done before it rewrites it
+    put();
+    named_bar_sync(1, 128);
+    if (tr) tr[5] = globaltimer_ns();
+    for (int e = wtid; e < G * D; e += 128) {
+        const int r = e / D, d = e % D;
+        float M = -INFINITY;
+#pragma unroll
+        for (int x = 0; x < 4; ++x) M = fmaxf(M, merge[(x * mrows + r) * (D + 2) + D]);
+        float L = 0.f, acc = 0.f;
+#pragma unroll
+        for (int x = 0; x < 4; ++x) {
+            const float* src = merge + (x * mrows + r) * (D + 2);
+            const float wgt = exp2f(src[D] - M);           // a warp pair that saw no key: m = -inf -> weight 0
+            L += src[D + 1] * wgt;
+            acc += src[d] * wgt;
+        }
+        if (w.nsplit == 1) {
+            const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r;
+            prm.out[orow * D + d] = __float2bfloat16_rn(acc / L);
+            if (prm.lse && d == 0) prm.lse[orow] = (M + log2f(L)) * kMLn2;
+        } else {
+            float* dst = prm.partials + ((int64_t)(w.partial + w.split) * G + r) * (D + 2);
+            dst[d] = acc;
+            if (d == 0) { dst[D] = M; dst[D + 1] = L; }
+        }
+    }
+    if (tr) tr[6] = globaltimer_ns();
+    // a5 hand-off: warp 3 publishes this split and, if it was the last of its (request, kv head), merges all of them; the
+    // decode warps go straight on to the next item.  mbarrier arrive = release at CTA scope for this thread's partial stores.
+    mbar_arrive(BAR(B_PARTIAL + slot));           // once per item and slot use (phase = slot use count)
+    named_bar_sync(1, 128);                       // every WG1 thread is done reading the merge buffer ...
+    named_bar_arrive(3, 256);                     // ... so WG2 may write the next decode item's partials
+}
+
+// a5: publish one decode split (acq_rel ticket) and, if it was the last of its (request, kv head), merge all splits in
+// fixed split order (bitwise reproducible).  One whole warp; `use` = how many times the scheduler slot has been used.
+template <int D>
+__device__ __forceinline__ void split_merge(const ss_work_item& w, const int slot, const uint32_t use, const int lane,
+                                            const uint32_t bar0, const MixParams& prm) {
+    auto BAR = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
+    const int Hq = prm.Hq, Hkv = prm.Hkv, G = Hq / Hkv;
+    mbar_wait(BAR(B_PARTIAL + slot), use & 1);   // acquire (CTA): all 128 merge threads' partial stores
+    int last = 0;
+    if (lane == 0) last = atom_add_acq_rel_gpu(prm.merge_counters + w.req * Hkv + w.head, 1) == w.nsplit - 1;
+    last = __shfl_sync(0xffffffffu, last, 0);
+    __syncwarp();
+    if (last) {
+        // lane owns columns d = lane + 32 j; 2 rows (q heads) per pass; per split 4 + 2 D/32 independent
+        // L2 loads in flight per lane (x2 unrolled), online log-sum-exp merge in split order
+        constexpr int DJ = D / 32;
+        const int64_t sstride = (int64_t)G * (D + 2);
+        const float* pbase = prm.partials + (int64_t)w.partial * sstride;
+        for (int r0 = 0; r0 < G; r0 += 2) {
+            float M[2], L[2], A[2][DJ];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                M[i] = -INFINITY; L[i] = 0.f;
+#pragma unroll
+                for (int j = 0; j < DJ; ++j) A[i][j] = 0.f;
+            }
+#pragma unroll 2
+            for (int x = 0; x < w.nsplit; ++x) {
+                const float* px = pbase + x * sstride;
+                float mx[2], lx[2], ox[2][DJ];
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const float* pr = px + min(r0 + i, G - 1) * (D + 2);
+                    mx[i] = __ldcg(pr + D);
+                    lx[i] = __ldcg(pr + D + 1);
+#pragma unroll
+                    for (int j = 0; j < DJ; ++j) ox[i][j] = __ldcg(pr + lane + 32 * j);
+                }
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const float Mn = fmaxf(M[i], mx[i]);
+                    const float al = exp2f(M[i] - Mn), bx = exp2f(mx[i] - Mn);
+                    L[i] = L[i] * al + lx[i] * bx;
+#pragma unroll
+                    for (int j = 0; j < DJ; ++j) A[i][j] = A[i][j] * al + ox[i][j] * bx;
+                    M[i] = Mn;
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                if (r0 + i < G) {
+                    const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r0 + i;
+                    const float inv = 1.f / L[i];
+#pragma unroll
+                    for (int j = 0; j < DJ; ++j) prm.out[orow * D + lane + 32 * j] = __float2bfloat16_rn(A[i][j] * inv);
+                    if (prm.lse && lane == 0) prm.lse[orow] = (M[i] + log2f(L[i])) * kMLn2;
+                }
+            }
+        }
+        if (lane == 0) prm.merge_counters[w.req * Hkv + w.head] = 0;     // re-armed for the next call
+    }
+}
+
 template <int D>
 __global__ void __launch_bounds__(kMixThreads, 1)
 mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
@@ -216,9 +541,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             mbar_init(BAR(B_KFULL + s), 1);
             mbar_init(BAR(B_VFULL + s), 1);
             mbar_init(BAR(B_KEMPTY_P + s), 2);               // one commit per chain
-            mbar_init(BAR(B_KEMPTY_D + s), 4);
+            mbar_init(BAR(B_KEMPTY_D + s), 8);               // every decode warp, every slot
             mbar_init(BAR(B_VEMPTY_P + s), 2);
-            mbar_init(BAR(B_VEMPTY_D + s), 4);
+            mbar_init(BAR(B_VEMPTY_D + s), 8);
         }
         for (int b = 0; b < 4; ++b) {
             mbar_init(BAR(B_SFULL + b), 1);
@@ -234,7 +559,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         for (int s = 0; s < kSchedSlots; ++s) {
             mbar_init(BAR(B_PARTIAL + s), 128);
             mbar_init(BAR(B_SCHED_FULL + s), 1);
-            mbar_init(BAR(B_SCHED_EMPTY + s), 10);               // 2 MMA warps + 8 worker warps
+            mbar_init(BAR(B_SCHED_EMPTY + s), 11);               // 2 MMA warps (warp 2 = a5) + the V producer + 8 worker warps
         }
         fence_barrier_init();
         prefetch_tmap(&tmap_q);
@@ -375,34 +700,19 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     const int s = tile_ctr % kNumSt;
                     const int npages = min(4, (w.kv_end - key0 + kPage - 1) / kPage);
                     const uint32_t bytes = (uint32_t)npages * kHalves * 2048;
-                    int crow[4];
+                    int cgrp[4];                                    // first 8-key group of the (page, kv head) slab
 #pragma unroll
-                    for (int p = 0; p < 4; ++p) crow[p] = (pg[p] * Hkv + g) * kPage;
+                    for (int p = 0; p < 4; ++p) cgrp[p] = (pg[p] * Hkv + g) * 2;
                     if (key0 + kSlotKeys < w.kv_end) load_pages(key0 + kSlotKeys);      // next tile's page ids in flight
                     const uint32_t lt = (lastT >> (2 * s)) & 3u;
                     const uint32_t epar = ((lt == 1 ? parP : parD) >> s) & 1u;
-                    // ---- K ----
+                    // K only: the V tiles of every item are streamed by warp 3 (one thread could not issue both: ~115 ns of
+                    // barrier round trip per phase + ~25 ns per TMA operation, ~600 ns per 32 KB tile = 52 GB/s per SM)
                     if (lt) mbar_wait(BAR((lt == 1 ? B_KEMPTY_P : B_KEMPTY_D) + s), epar);
                     mbar_arrive_expect_tx(BAR(B_KFULL + s), bytes);
 #pragma unroll
                     for (int p = 0; p < 4; ++p)
-                        if (p < npages) {
-#pragma unroll
-                            for (int hh = 0; hh < kHalves; ++hh)
-                                tma_load_2d(sbase + SM::kKOff + s * SM::kSlot + hh * (kSlotKeys * 128) + p * (kPage * 128),
-                                            &tmap_k, hh * 64, crow[p], BAR(B_KFULL + s));
-                        }
-                    // ---- V ----
-                    if (lt) mbar_wait(BAR((lt == 1 ? B_VEMPTY_P : B_VEMPTY_D) + s), epar);
-                    mbar_arrive_expect_tx(BAR(B_VFULL + s), bytes);
-#pragma unroll
-                    for (int p = 0; p < 4; ++p)
-                        if (p < npages) {
-#pragma unroll
-                            for (int hh = 0; hh < kHalves; ++hh)
-                                tma_load_2d(sbase + SM::kVOff + s * SM::kSlot + hh * (kSlotKeys * 128) + p * (kPage * 128),
-                                            &tmap_v, hh * 64, crow[p], BAR(B_VFULL + s));
-                        }
+                        if (p < npages) tma_load_slab(sbase + SM::kKOff + s * SM::kSlot + p * SM::kPageBytes, &tmap_k, cgrp[p], BAR(B_KFULL + s));
                     if (lt == 1) parP ^= 1u << s; else if (lt == 2) parD ^= 1u << s;
                     lastT = (lastT & ~(3u << (2 * s))) | ((uint32_t)w.kind << (2 * s));
                 }
@@ -417,14 +727,54 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 }
             }
         }
-      } else if (warp <= 2) {
+      } else if (warp == 3) {
+        // =============================== V producer ===============================
+        // Follows the scheduler ring like every consumer and streams the V tiles of each item into the V ring: same slot
+        // order and the same typed-EMPTY bookkeeping as warp 0 keeps for K.  One elected thread, waits included.
+        if (elect_one()) {
+            uint32_t parP = 0, parD = 0, lastT = 0, tile_ctr = 0, n_sched = 0;
+            for (;;) {
+                const int slot = n_sched % kSchedSlots;
+                mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
+                const ss_work_item w = sched[slot];
+                ++n_sched;
+                if (w.kind == 0) break;
+                const int32_t* bt = prm.block_table + (int64_t)w.req * prm.max_pages;
+                const int g = w.kind == 1 ? w.head / G : w.head;
+                int pg[4];
+                auto load_pages = [&](int key0) {
+#pragma unroll
+                    for (int p = 0; p < 4; ++p) pg[p] = (key0 + p * kPage < w.kv_end) ? __ldg(bt + (key0 >> 4) + p) : 0;
+                };
+                load_pages(w.kv_begin);
+                for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kSlotKeys, ++tile_ctr) {
+                    const int s = tile_ctr % kNumSt;
+                    const int npages = min(4, (w.kv_end - key0 + kPage - 1) / kPage);
+                    int cgrp[4];
+#pragma unroll
+                    for (int p = 0; p < 4; ++p) cgrp[p] = (pg[p] * Hkv + g) * 2;
+                    if (key0 + kSlotKeys < w.kv_end) load_pages(key0 + kSlotKeys);      // next tile's page ids in flight
+                    const uint32_t lt = (lastT >> (2 * s)) & 3u;
+                    const uint32_t epar = ((lt == 1 ? parP : parD) >> s) & 1u;
+                    if (lt) mbar_wait(BAR((lt == 1 ? B_VEMPTY_P : B_VEMPTY_D) + s), epar);
+                    mbar_arrive_expect_tx(BAR(B_VFULL + s), (uint32_t)npages * SM::kPageBytes);
+#pragma unroll
+                    for (int p = 0; p < 4; ++p)
+                        if (p < npages) tma_load_slab(sbase + SM::kVOff + s * SM::kSlot + p * SM::kPageBytes, &tmap_v, cgrp[p], BAR(B_VFULL + s));
+                    if (lt == 1) parP ^= 1u << s; else if (lt == 2) parD ^= 1u << s;
+                    lastT = (lastT & ~(3u << (2 * s))) | ((uint32_t)w.kind << (2 * s));
+                }
+                mbar_arrive(BAR(B_SCHED_EMPTY + slot));
+            }
+        }
+      } else {
         // =============================== tcgen05.mma issuers ===============================
         // Warp 1 issues chain A's MMAs, warp 2 chain B's (one elected thread each, waits included, so descriptors stay
         // in uniform registers).  Two issuers because one thread could not keep the pipe fed: per (chain, half tile)
         // it spent ~250 cycles in three mbarrier round trips and ~740 blocked in issue (profiles/r2_a3.md), serially
         // for both chains.  The chains touch disjoint TMEM and only read the shared K/V slots, so no order is needed
         // between them; the slot / Q-tile release barriers take one commit per chain (chain A commits twice when the
-        // item has a single head).  Decode items: nothing to do here (a5 runs on WG2).
+        // item has a single head).  Decode items: warp 1 has nothing to do, warp 2 runs a5 (split_merge).
         constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kSlotKeys, 0);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileRows, D, 1);
         const int X = warp - 1;
@@ -453,12 +803,12 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         tc_fence_after();
                         SS_MM(1)
                         const uint64_t qdesc0 = umma_desc_sw128(sbase + SM::kQOff + X * SM::kQTile, 16, 1024);
-                        const uint64_t kdesc0 = umma_desc_sw128(sbase + SM::kKOff + s * SM::kSlot, 16, 1024);
+                        const uint64_t kdesc0 = umma_desc_sw128(sbase + SM::kKOff + s * SM::kSlot, 16, SM::kGroup);
 #pragma unroll
                         for (int ks = 0; ks < D / 16; ++ks) {
                             // bytes; descriptor address unit = 16 B.  64-column halves: Q 128 rows, K 64 rows apart
                             const uint32_t qoff = (ks >> 2) * (kTileRows * 128) + (ks & 3) * 32;
-                            const uint32_t koff = (ks >> 2) * (kSlotKeys * 128) + (ks & 3) * 32;
+                            const uint32_t koff = (ks >> 2) * 1024 + (ks & 3) * 32;
                             umma_ss(tchain + b * 64, qdesc0 + (qoff >> 4), kdesc0 + (koff >> 4), idesc_qk, ks > 0);
                         }
                         umma_commit(BAR(B_SFULL + X * 2 + b));
@@ -474,10 +824,10 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
                         tc_fence_after();
                         SS_MM(1)
-                        const uint64_t vdesc0 = umma_desc_sw128(sbase + SM::kVOff + s * SM::kSlot, kSlotKeys * 128, 1024);
+                        const uint64_t vdesc0 = umma_desc_sw128(sbase + SM::kVOff + s * SM::kSlot, 1024, SM::kGroup);   // halves 1024 apart, 8-key groups kGroup
 #pragma unroll
                         for (int kk = 0; kk < kSlotKeys / 16; ++kk)      // A = P[b] from TMEM: 16 keys = 8 packed columns
-                            umma_ts(tchain + SM::kTmemO, tchain + b * 64 + kk * 8, vdesc0 + (uint64_t)(kk * 2048 >> 4), idesc_pv, (kt > 0 || kk > 0));
+                            umma_ts(tchain + SM::kTmemO, tchain + b * 64 + kk * 8, vdesc0 + (uint64_t)(kk * SM::kPageBytes >> 4), idesc_pv, (kt > 0 || kk > 0));
                         umma_commit(BAR(B_PVDONE + X));
                         for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_VEMPTY_P + s));
                         if (kt == n - 1) {
@@ -509,30 +859,30 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 __syncwarp();
                 if (X < nq) { s_ctr += n; ++n_chain; }
                 ++n_pre;
+            } else if (X == 1 && w.nsplit > 1) {
+                split_merge<D>(w, slot, (n_sched - 1) / kSchedSlots, lane, bar0, prm);
             }
             tile_ctr += n;
             __syncwarp();
             if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
         }
-        if (trace && lane == 0 && X == 0) trace[4] = globaltimer_ns();
+        if (trace && lane == 0 && X == 1) trace[4] = globaltimer_ns();
       }
     } else {
         setmaxnreg_inc<kRegsWorker>();
         // =============================== workers ===============================
-        const int wg = (warp - 4) >> 2;                        // 0: chain A / decode, 1: chain B / a5 merge
-        const int cw = (warp - 4) & 3;                         // decode: key slice
+        const int wg = (warp - 4) >> 2;                        // 0: chain A / decode on even slots, 1: chain B / decode on odd slots
+        const int cw = (warp - 4) & 3;                         // decode: 16-key slice of the slot
         const int quarter = warp & 3;                          // TMEM lane quarter this warp may access
         const int row = quarter * 32 + lane;                   // prefill: query row inside the tile
         const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
         const int wtid = threadIdx.x - 128 - wg * 128;         // 0..127 inside the warpgroup
         const float sl2 = prm.scale * kMLog2e;
-        const int qrow = lane >> 2, qcol = (lane & 3) * 2;     // mma.sync fragment coordinates
         const uint32_t tchain = tmem_base + wg * SM::kTmemChain;
         const uint32_t tmem_o = tchain + SM::kTmemO;
         uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_chain = 0;
         float* merge = reinterpret_cast<float*>(smem + SM::kQOff);
-        const bool q_staged = G <= 8;
-        const int mrows = q_staged ? 8 : kMaxGroup;           // merge-buffer rows per warp
+        if (wg == 0) named_bar_arrive(3, 256);                 // the decode merge buffer starts out free (see stage A below)
         for (;;) {
             const int slot = n_sched % kSchedSlots;
             mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
@@ -573,7 +923,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         for (int i = wtid; i < (kSlotKeys - first) * kHalves * 8; i += 128) {
                             const int r = first + i / (kHalves * 8);
                             const int c = i % (kHalves * 8);
-                            const uint32_t a = vaddr + (c >> 3) * (kSlotKeys * 128) + r * 128 + (c & 7) * 16;
+                            const uint32_t a = vaddr + SM::kv_off(r, c);
                             asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
                         }
                     }
@@ -655,235 +1005,17 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 ++n_chain;
             } else if (w.kind == 1) {
                 // single-head item: chain B has nothing to do
-            } else if (wg == 0) {
-                // -------------------------- decode split: warp = 32-key slice of a pair of 64-key slots --------------------------
-                uint32_t qa[D / 16][4];
-                if (q_staged) {
-                    const uint32_t qs = sbase + SM::kQStageOff + slot * SM::kQStageBytes + (qrow * D + qcol) * 2;
-#pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks) {
-                        qa[ks][0] = qrow < G ? lds32(qs + ks * 32) : 0u;
-                        qa[ks][2] = qrow < G ? lds32(qs + ks * 32 + 16) : 0u;
-                        qa[ks][1] = 0u;
-                        qa[ks][3] = 0u;
-                    }
-                } else {
-                    const __nv_bfloat16* qb = prm.q + ((int64_t)w.row0 * Hq + (int64_t)w.head * G) * D;
-#pragma unroll
-                    for (int ks = 0; ks < D / 16; ++ks) {
-                        const int d0 = ks * 16 + qcol;
-                        qa[ks][0] = qrow < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)qrow * D + d0) : 0u;
-                        qa[ks][1] = qrow + 8 < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)(qrow + 8) * D + d0) : 0u;
-                        qa[ks][2] = qrow < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)qrow * D + d0 + 8) : 0u;
-                        qa[ks][3] = qrow + 8 < G ? *reinterpret_cast<const uint32_t*>(qb + (int64_t)(qrow + 8) * D + d0 + 8) : 0u;
-                    }
-                }
-                float o[D / 8][4];
-#pragma unroll
-                for (int i = 0; i < D / 8; ++i) o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f;
-                float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
-                // Warps 0,1 compute on the even slots of the item, warps 2,3 on the odd ones (32 rows each), but EVERY warp
-                // waits FULL and arrives EMPTY on EVERY slot: an mbarrier parity wait is only sound while the waiter is
-                // less than one phase away from the barrier, and with 5 ring slots a slot alternates between the pairs.
-                const int sub = cw >> 1, r32 = (cw & 1) * 32;      // which slot of the pair, which 32 rows of it
-                for (int t = 0; t < n; ++t) {
-                    const uint32_t tc = tile_ctr + t;
-                    const int s = tc % kNumSt;
-                    const uint32_t fpar = (tc / kNumSt) & 1;
-                    const int key0 = w.kv_begin + t * kSlotKeys;
-                    const int nvalid = (t & 1) == sub ? w.kv_end - (key0 + r32) : 0;      // 0: not this warp's slot
-                    const uint32_t kbase = sbase + SM::kKOff + s * SM::kSlot;
-                    const uint32_t vbase = sbase + SM::kVOff + s * SM::kSlot;
-                    float sacc[4][4];
-                    mbar_wait(BAR(B_KFULL + s), fpar);
-                    if (tr && t == 0) tr[3] = globaltimer_ns();
-                    if (nvalid > 0) {
-#pragma unroll
-                        for (int nt = 0; nt < 4; ++nt) sacc[nt][0] = sacc[nt][1] = sacc[nt][2] = sacc[nt][3] = 0.f;
-#pragma unroll
-                        for (int j = 0; j < D / 32; ++j) {
-#pragma unroll
-                            for (int nt = 0; nt < 4; ++nt) {
-                                const int r = r32 + nt * 8 + (lane & 7);
-                                const int cd = 4 * j + (lane >> 3);
-                                const uint32_t a = kbase + (cd >> 3) * (kSlotKeys * 128) + r * 128 + (((cd & 7) ^ (r & 7)) << 4);
-                                uint32_t b0, b1, b2, b3;
-                                ldmatrix_x4(b0, b1, b2, b3, a);
-                                mma_bf16_16816(sacc[nt], qa[2 * j], b0, b1);
-                                mma_bf16_16816(sacc[nt], qa[2 * j + 1], b2, b3);
-                            }
-                        }
-                    }
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(BAR(B_KEMPTY_D + s));
-                    mbar_wait(BAR(B_VFULL + s), fpar);
-                    if (nvalid > 0) {
-                        if (nvalid < 32) {
-                            for (int i = lane; i < (32 - nvalid) * kHalves * 8; i += 32) {
-                                const int r = r32 + nvalid + i / (kHalves * 8);
-                                const int c = i % (kHalves * 8);
-                                const uint32_t a = vbase + (c >> 3) * (kSlotKeys * 128) + r * 128 + (c & 7) * 16;
-                                asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
-                            }
-                            __syncwarp();
-                        }
-                        float bm0 = -INFINITY, bm1 = -INFINITY;
-#pragma unroll
-                        for (int nt = 0; nt < 4; ++nt) {
-                            const int c = nt * 8 + qcol;
-                            if (c >= nvalid) { sacc[nt][0] = -INFINITY; sacc[nt][2] = -INFINITY; }
-                            if (c + 1 >= nvalid) { sacc[nt][1] = -INFINITY; sacc[nt][3] = -INFINITY; }
-                            bm0 = fmaxf(bm0, fmaxf(sacc[nt][0], sacc[nt][1]));
-                            bm1 = fmaxf(bm1, fmaxf(sacc[nt][2], sacc[nt][3]));
-                        }
-                        bm0 = fmaxf(bm0, __shfl_xor_sync(0xffffffffu, bm0, 1));
-                        bm0 = fmaxf(bm0, __shfl_xor_sync(0xffffffffu, bm0, 2));
-                        bm1 = fmaxf(bm1, __shfl_xor_sync(0xffffffffu, bm1, 1));
-                        bm1 = fmaxf(bm1, __shfl_xor_sync(0xffffffffu, bm1, 2));
-                        const float mn0 = fmaxf(m0, bm0 * sl2), mn1 = fmaxf(m1, bm1 * sl2);
-                        const float al0 = exp2f(m0 - mn0), al1 = exp2f(m1 - mn1);
-                        float ps0 = 0.f, ps1 = 0.f;
-                        uint32_t pa[2][4];
-#pragma unroll
-                        for (int nt = 0; nt < 4; ++nt) {
-                            const float p0 = exp2f(sacc[nt][0] * sl2 - mn0), p1 = exp2f(sacc[nt][1] * sl2 - mn0);
-                            const float p2 = exp2f(sacc[nt][2] * sl2 - mn1), p3 = exp2f(sacc[nt][3] * sl2 - mn1);
-                            ps0 += p0 + p1;
-                            ps1 += p2 + p3;
-                            pa[nt >> 1][(nt & 1) * 2 + 0] = pack_bf16(p0, p1);
-                            pa[nt >> 1][(nt & 1) * 2 + 1] = pack_bf16(p2, p3);
-                        }
-                        l0 = l0 * al0 + ps0;
-                        l1 = l1 * al1 + ps1;
-                        m0 = mn0;
-                        m1 = mn1;
-#pragma unroll
-                        for (int i = 0; i < D / 8; ++i) { o[i][0] *= al0; o[i][1] *= al0; o[i][2] *= al1; o[i][3] *= al1; }
-#pragma unroll
-                        for (int kk = 0; kk < 2; ++kk) {
-#pragma unroll
-                            for (int np = 0; np < D / 16; ++np) {
-                                const int r = r32 + kk * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
-                                const int cd = 2 * np + (lane >> 4);
-                                const uint32_t a = vbase + (cd >> 3) * (kSlotKeys * 128) + r * 128 + (((cd & 7) ^ (r & 7)) << 4);
-                                uint32_t b0, b1, b2, b3;
-                                ldmatrix_x4_trans(b0, b1, b2, b3, a);
-                                mma_bf16_16816(o[2 * np], pa[kk], b0, b1);
-                                mma_bf16_16816(o[2 * np + 1], pa[kk], b2, b3);
-                            }
-                        }
-                        if (nvalid < 32) fence_proxy_async();
-                    }
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(BAR(B_VEMPTY_D + s));
-                }
-                // ---- cross-warp log-sum-exp merge through smem ----
-                if (tr) tr[4] = globaltimer_ns();
-                l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
-                l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
-                l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
-                l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
-                float* mine = merge + cw * mrows * (D + 2);
-#pragma unroll
-                for (int i = 0; i < D / 8; ++i) {
-                    *reinterpret_cast<float2*>(mine + qrow * (D + 2) + i * 8 + qcol) = make_float2(o[i][0], o[i][1]);
-                    if (!q_staged) *reinterpret_cast<float2*>(mine + (qrow + 8) * (D + 2) + i * 8 + qcol) = make_float2(o[i][2], o[i][3]);
-                }
-                if ((lane & 3) == 0) {
-                    mine[qrow * (D + 2) + D] = m0;
-                    mine[qrow * (D + 2) + D + 1] = l0;
-                    if (!q_staged) {
-                        mine[(qrow + 8) * (D + 2) + D] = m1;
-                        mine[(qrow + 8) * (D + 2) + D + 1] = l1;
-                    }
-                }
-                named_bar_sync(1, 128);
-                if (tr) tr[5] = globaltimer_ns();
-                for (int e = wtid; e < G * D; e += 128) {
-                    const int r = e / D, d = e % D;
-                    float M = -INFINITY;
-#pragma unroll
-                    for (int x = 0; x < 4; ++x) M = fmaxf(M, merge[(x * mrows + r) * (D + 2) + D]);
-                    float L = 0.f, acc = 0.f;
-#pragma unroll
-                    for (int x = 0; x < 4; ++x) {
-                        const float* src = merge + (x * mrows + r) * (D + 2);
-                        const float wgt = exp2f(src[D] - M);           // a warp that saw no key: m = -inf -> weight 0
-                        L += src[D + 1] * wgt;
-                        acc += src[d] * wgt;
-                    }
-                    if (w.nsplit == 1) {
-                        const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r;
-                        prm.out[orow * D + d] = __float2bfloat16_rn(acc / L);
-                        if (prm.lse && d == 0) prm.lse[orow] = (M + log2f(L)) * kMLn2;
-                    } else {
-                        float* dst = prm.partials + ((int64_t)(w.partial + w.split) * G + r) * (D + 2);
-                        dst[d] = acc;
-                        if (d == 0) { dst[D] = M; dst[D + 1] = L; }
-                    }
-                }
-                if (tr) tr[6] = globaltimer_ns();
-                // a5 hand-off: WG2 publishes this split and, if it was the last of its (request, kv head), merges all
-                // of them; the decode warps go straight on to the next item.  mbarrier arrive = release at CTA scope
-                // for this thread's partial stores.
-                mbar_arrive(BAR(B_PARTIAL + slot));           // once per item and slot use (phase = slot use count)
-                named_bar_sync(1, 128);                       // merge buffer free for the next item
-            } else if (cw == 0 && w.nsplit > 1) {
-                // ---- a5 (WG2 warp 0): publish this split; the last ticket of (request, kv head) merges in fixed split order ----
-                mbar_wait(BAR(B_PARTIAL + slot), ((n_sched - 1) / kSchedSlots) & 1);   // acquire (CTA): all 128 decode threads' partial stores
-                int last = 0;
-                if (lane == 0) last = atom_add_acq_rel_gpu(prm.merge_counters + w.req * Hkv + w.head, 1) == w.nsplit - 1;
-                last = __shfl_sync(0xffffffffu, last, 0);
-                __syncwarp();
-                if (last) {
-                    // lane owns columns d = lane + 32 j; 4 rows (q heads) per pass; per split 8 + 4 D/32 independent
-                    // L2 loads in flight per lane, online log-sum-exp merge in split order
-                    constexpr int DJ = D / 32;
-                    const int64_t sstride = (int64_t)G * (D + 2);
-                    const float* pbase = prm.partials + (int64_t)w.partial * sstride;
-                    for (int r0 = 0; r0 < G; r0 += 4) {
-                        float M[4], L[4], A[4][DJ];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            M[i] = -INFINITY; L[i] = 0.f;
-#pragma unroll
-                            for (int j = 0; j < DJ; ++j) A[i][j] = 0.f;
-                        }
-#pragma unroll 2
-                        for (int x = 0; x < w.nsplit; ++x) {
-                            const float* px = pbase + x * sstride;
-                            float mx[4], lx[4], ox[4][DJ];
-#pragma unroll
-                            for (int i = 0; i < 4; ++i) {
-                                const float* pr = px + min(r0 + i, G - 1) * (D + 2);
-                                mx[i] = __ldcg(pr + D);
-                                lx[i] = __ldcg(pr + D + 1);
-#pragma unroll
-                                for (int j = 0; j < DJ; ++j) ox[i][j] = __ldcg(pr + lane + 32 * j);
-                            }
-#pragma unroll
-                            for (int i = 0; i < 4; ++i) {
-                                const float Mn = fmaxf(M[i], mx[i]);
-                                const float al = exp2f(M[i] - Mn), bx = exp2f(mx[i] - Mn);
-                                L[i] = L[i] * al + lx[i] * bx;
-#pragma unroll
-                                for (int j = 0; j < DJ; ++j) A[i][j] = A[i][j] * al + ox[i][j] * bx;
-                                M[i] = Mn;
-                            }
-                        }
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) {
-                            if (r0 + i < G) {
-                                const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r0 + i;
-                                const float inv = 1.f / L[i];
-#pragma unroll
-                                for (int j = 0; j < DJ; ++j) prm.out[orow * D + lane + 32 * j] = __float2bfloat16_rn(A[i][j] * inv);
-                                if (prm.lse && lane == 0) prm.lse[orow] = (M[i] + log2f(L[i])) * kMLn2;
-                            }
-                        }
-                    }
-                    if (lane == 0) prm.merge_counters[w.req * Hkv + w.head] = 0;     // re-armed for the next call
-                }
+            } else {
+                // -------------------------- decode split: all 8 worker warps --------------------------
+                // Warp dw owns 16 keys of every other 64-key slot: warps 0-3 (WG1) the even slots of the item, warps 4-7
+                // (WG2) the odd ones.  The products are taken TRANSPOSED, keys on the M = 16 side of mma.sync.m16n8k16
+                // and the G query heads of the KV head on the N = 8 side:  S^T = K Q^T  (A = K rows from smem by
+                // ldmatrix, B = Q^T from the staged Q rows),  O^T += V^T P^T  (A = V by ldmatrix.trans, B = P^T by
+                // movmatrix from the S^T accumulators).  With heads padded to M = 16 instead, a 64-key tile cost 128 HMMA
+                // and the legacy tensor path (~1 HMMA.16816 per 9 clk and SM) capped an SM at ~52 GB/s whatever the
+                // ring depth, copy mechanism or warp count (profiles/r2b.md); this form needs 64 (G <= 8).
+                if (G <= 8) decode_item<D, 1>(w, n, slot, tile_ctr, wg, cw, lane, wtid, sbase, bar0, prm, merge, tr);
+                else        decode_item<D, 2>(w, n, slot, tile_ctr, wg, cw, lane, wtid, sbase, bar0, prm, merge, tr);
             }
             tile_ctr += n;
             if (tr) tr[1] = globaltimer_ns();
