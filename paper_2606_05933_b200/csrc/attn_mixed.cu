@@ -4,7 +4,7 @@
 // Persistent CTAs (one per SM) pull items from the device work list through a dynamic queue (atomic
 // counter), so tensor-bound prefill tiles and HBM-bound decode splits overlap across SMs and the batch
 // costs ~max(bytes/HBM, flops/tensor) instead of the sum.  12 warps per CTA in 3 warpgroups; the register
-// file is re-partitioned with setmaxnreg (WG0 72 registers per thread, WG1 / WG2 216):
+// file is re-partitioned with setmaxnreg (WG0 88 registers per thread, WG1 / WG2 208):
 //   WG0 warp 0  scheduler + Q / K producer (one elected thread).  Publishes each item to the other warps through a
 //               4-slot smem ring, loads the Q tiles (prefill: the item's 1 or 2 query heads, 128 rows each) and
 //               streams 64-key K tiles into a 5-slot K ring: ONE 4-D TMA box per (page, kv head) slab (16 keys x D,
@@ -62,8 +62,9 @@ constexpr int kNumSt = SS_NUM_ST;    // K ring slots = V ring slots
 constexpr int kSchedSlots = 4;
 constexpr int kDecKeys = 16;         // keys of a 64-key slot one decode warp owns (4 warps per slot)
 // setmaxnreg moves registers inside the CTA's own launch allocation: 384 threads x 168 (the __launch_bounds__ cap ptxas
-// reports) = 64512, so 128*72 + 256*216 = 64512 fits exactly; one register more per worker and the .inc spins forever.
-constexpr int kRegsLaunch = 168, kRegsWg0 = 72, kRegsWorker = 216;
+// reports) = 64512, so 128*88 + 256*208 = 64512 fits exactly; one register more per worker and the .inc spins forever.
+// (88: the K producer thread keeps the next item, three tiles of page ids and its slot history without spilling.)
+constexpr int kRegsLaunch = 168, kRegsWg0 = 88, kRegsWorker = 208;
 static_assert(128 * kRegsWg0 + 256 * kRegsWorker <= kMixThreads * kRegsLaunch, "setmaxnreg.inc could never be granted");
 constexpr float kMLog2e = 1.4426950408889634f;
 constexpr float kMLn2 = 0.6931471805599453f;
@@ -453,6 +454,76 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
     named_bar_arrive(3, 256);                     // ... so WG2 may write the next decode item's partials
 }
 
+// One tensor's tile stream (K by warp 0, V by warp 3), run by ONE thread: 64-key tiles of an item's KV range into the
+// ring, one 4-D TMA box per (page, kv head) slab.  What the loop is shaped around (measured, profiles/r2b.md): the thread
+// pays ~115 ns per barrier phase (try_wait round trip + arrive.expect_tx) and ~25 ns per TMA operation whose
+// coordinates must first reach uniform registers (LDG -> IMAD -> R2UR).  So: the EMPTY test of the NEXT slot is issued
+// before this tile's operations (its round trip overlaps them), full tiles take a branch-free path so the four R2UR /
+// UTMALDG pairs can be scheduled together, and page ids are loaded two tiles ahead of their use.
+// Slot history as bit fields: parity of the next EMPTY wait per consumer type, and the type (1 prefill / 2 decode) of
+// the slot's last consumer, which names the EMPTY barrier that consumer will arrive on.
+template <int D, int B_FULL0, int B_EMPTY_P0, int B_EMPTY_D0>
+struct TileStreamer {
+    using SM = MixSmem<D>;
+    uint32_t parP = 0, parD = 0, lastT = 0;
+    int s = 0;                     // ring slot of the next tile
+    uint32_t eb = 0, epar = 0;     // EMPTY barrier (0: slot never used) and parity the next tile must see
+    bool ok = true;                // ... and whether an early test already found it complete
+    uint32_t bar0, ring;           // shared addresses: barrier block, this tensor's ring
+    const CUtensorMap* tmap;
+
+    __device__ __forceinline__ uint32_t BAR(int i) const { return bar0 + 8u * (uint32_t)i; }
+    __device__ __forceinline__ void look(int slot, uint32_t& b, uint32_t& par) const {
+        const uint32_t lt = (lastT >> (2 * slot)) & 3u;
+        par = ((lt == 1 ? parP : parD) >> slot) & 1u;
+        b = lt ? BAR((lt == 1 ? B_EMPTY_P0 : B_EMPTY_D0) + slot) : 0u;
+    }
+    // streams keys [w.kv_begin, w.kv_end) of request row `bt`, kv head g; pg = page ids of the first tile;
+    // on_last() runs just before the item's last tile is issued
+    template <typename F>
+    __device__ __forceinline__ void item(const ss_work_item& w, const int32_t* __restrict__ bt, const int g, const int Hkv,
+                                         int (&pg)[4], F on_last) {
+        auto load_pages = [&](int key0, int (&dst)[4]) {
+#pragma unroll
+            for (int p = 0; p < 4; ++p) dst[p] = (key0 + p * kPage < w.kv_end) ? __ldg(bt + (key0 >> 4) + p) : 0;
+        };
+        int pg1[4];
+        load_pages(w.kv_begin + kSlotKeys, pg1);
+        for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kSlotKeys) {
+            if (key0 + kSlotKeys >= w.kv_end) on_last();
+            int pg2[4];
+            load_pages(key0 + 2 * kSlotKeys, pg2);                 // used two iterations from now
+            int cg[4];                                             // first 8-key group of each (page, kv head) slab
+#pragma unroll
+            for (int p = 0; p < 4; ++p) cg[p] = (pg[p] * Hkv + g) * 2;
+            const int s1 = s + 1 == kNumSt ? 0 : s + 1;
+            uint32_t eb1, epar1;
+            look(s1, eb1, epar1);                                  // slot s1's history cannot change while tile s is issued
+            while (!ok) ok = mbar_try_wait(eb, epar);
+            const bool ok1 = eb1 ? mbar_try_wait(eb1, epar1) : true;   // early test: its round trip overlaps the issue below
+            const uint32_t full = BAR(B_FULL0 + s), dst = ring + s * SM::kSlot;
+            const int nkeys = w.kv_end - key0;
+            if (nkeys >= kSlotKeys) {
+                mbar_arrive_expect_tx(full, 4u * SM::kPageBytes);
+#pragma unroll
+                for (int p = 0; p < 4; ++p) tma_load_slab(dst + p * SM::kPageBytes, tmap, cg[p], full);
+            } else {
+                const int npages = (nkeys + kPage - 1) / kPage;
+                mbar_arrive_expect_tx(full, (uint32_t)npages * SM::kPageBytes);
+#pragma unroll
+                for (int p = 0; p < 4; ++p)
+                    if (p < npages) tma_load_slab(dst + p * SM::kPageBytes, tmap, cg[p], full);
+            }
+            const uint32_t lt = (lastT >> (2 * s)) & 3u;
+            if (lt == 1) parP ^= 1u << s; else if (lt == 2) parD ^= 1u << s;
+            lastT = (lastT & ~(3u << (2 * s))) | ((uint32_t)w.kind << (2 * s));
+            s = s1; eb = eb1; epar = epar1; ok = ok1;
+#pragma unroll
+            for (int p = 0; p < 4; ++p) { pg[p] = pg1[p]; pg1[p] = pg2[p]; }
+        }
+    }
+};
+
 // a5: publish one decode split (acq_rel ticket) and, if it was the last of its (request, kv head), merge all splits in
 // fixed split order (bitwise reproducible).  One whole warp; `use` = how many times the scheduler slot has been used.
 template <int D>
@@ -610,8 +681,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             int32_t* const q_pre = prm.queue, * const q_dec = prm.queue + 1;
             bool pre_done = n_pre_items == 0, dec_done = n_dec == 0;
             // per-slot history as bit fields: parity of the next EMPTY wait per consumer type, last consumer type
-            uint32_t parP = 0, parD = 0, lastT = 0;
-            uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0;
+            TileStreamer<D, B_KFULL, B_KEMPTY_P, B_KEMPTY_D> ks;
+            ks.bar0 = bar0; ks.ring = sbase + SM::kKOff; ks.tmap = &tmap_k;
+            uint32_t n_sched = 0, n_pre = 0;
             int prev_kind = 0;
             const bool q_staged = G <= 8;
             union WU { ss_work_item it; uint4 v[3]; };
@@ -670,10 +742,6 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 int pg[4];
 #pragma unroll
                 for (int p = 0; p < 4; ++p) pg[p] = nxt_pg[p];
-                auto load_pages = [&](int key0) {
-#pragma unroll
-                    for (int p = 0; p < 4; ++p) pg[p] = (key0 + p * kPage < w.kv_end) ? __ldg(bt + (key0 >> 4) + p) : 0;
-                };
                 if (w.kind == 1) {
                     mbar_wait(BAR(B_QEMPTY), (n_pre & 1) ^ 1);
                     if (prev_kind == 2) {
@@ -690,32 +758,13 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     ++n_pre;
                 }
                 prev_kind = w.kind;
-                for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kSlotKeys, ++tile_ctr) {
-                    if (key0 + kSlotKeys >= w.kv_end) {
-                        // last tile of this item: draw the next ticket now (not earlier, or the tail of the launch
-                        // grows by an item held while this one is still streaming); the ring hides the chain
-                        fetch(nxt);
-                        first_pages(nxt.it, nxt_pg);
-                    }
-                    const int s = tile_ctr % kNumSt;
-                    const int npages = min(4, (w.kv_end - key0 + kPage - 1) / kPage);
-                    const uint32_t bytes = (uint32_t)npages * kHalves * 2048;
-                    int cgrp[4];                                    // first 8-key group of the (page, kv head) slab
-#pragma unroll
-                    for (int p = 0; p < 4; ++p) cgrp[p] = (pg[p] * Hkv + g) * 2;
-                    if (key0 + kSlotKeys < w.kv_end) load_pages(key0 + kSlotKeys);      // next tile's page ids in flight
-                    const uint32_t lt = (lastT >> (2 * s)) & 3u;
-                    const uint32_t epar = ((lt == 1 ? parP : parD) >> s) & 1u;
-                    // K only: the V tiles of every item are streamed by warp 3 (one thread could not issue both: ~115 ns of
-                    // barrier round trip per phase + ~25 ns per TMA operation, ~600 ns per 32 KB tile = 52 GB/s per SM)
-                    if (lt) mbar_wait(BAR((lt == 1 ? B_KEMPTY_P : B_KEMPTY_D) + s), epar);
-                    mbar_arrive_expect_tx(BAR(B_KFULL + s), bytes);
-#pragma unroll
-                    for (int p = 0; p < 4; ++p)
-                        if (p < npages) tma_load_slab(sbase + SM::kKOff + s * SM::kSlot + p * SM::kPageBytes, &tmap_k, cgrp[p], BAR(B_KFULL + s));
-                    if (lt == 1) parP ^= 1u << s; else if (lt == 2) parD ^= 1u << s;
-                    lastT = (lastT & ~(3u << (2 * s))) | ((uint32_t)w.kind << (2 * s));
-                }
+                // K only: the V tiles of every item are streamed by warp 3 (one thread could not issue both).  At the item's
+                // last tile the next ticket is drawn (not earlier, or the tail of the launch grows by an item held while
+                // this one is still streaming); the ring hides the atomic -> record -> block-table chain.
+                ks.item(w, bt, g, Hkv, pg, [&]() {
+                    fetch(nxt);
+                    first_pages(nxt.it, nxt_pg);
+                });
             }
             if (prm.self_plan) {
                 // self-cleaning queue: every CTA checks out after its last ticket; the last one re-arms the counters
@@ -732,7 +781,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         // Follows the scheduler ring like every consumer and streams the V tiles of each item into the V ring: same slot
         // order and the same typed-EMPTY bookkeeping as warp 0 keeps for K.  One elected thread, waits included.
         if (elect_one()) {
-            uint32_t parP = 0, parD = 0, lastT = 0, tile_ctr = 0, n_sched = 0;
+            TileStreamer<D, B_VFULL, B_VEMPTY_P, B_VEMPTY_D> vs;
+            vs.bar0 = bar0; vs.ring = sbase + SM::kVOff; vs.tmap = &tmap_v;
+            uint32_t n_sched = 0;
             for (;;) {
                 const int slot = n_sched % kSchedSlots;
                 mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
@@ -742,28 +793,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 const int32_t* bt = prm.block_table + (int64_t)w.req * prm.max_pages;
                 const int g = w.kind == 1 ? w.head / G : w.head;
                 int pg[4];
-                auto load_pages = [&](int key0) {
 #pragma unroll
-                    for (int p = 0; p < 4; ++p) pg[p] = (key0 + p * kPage < w.kv_end) ? __ldg(bt + (key0 >> 4) + p) : 0;
-                };
-                load_pages(w.kv_begin);
-                for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kSlotKeys, ++tile_ctr) {
-                    const int s = tile_ctr % kNumSt;
-                    const int npages = min(4, (w.kv_end - key0 + kPage - 1) / kPage);
-                    int cgrp[4];
-#pragma unroll
-                    for (int p = 0; p < 4; ++p) cgrp[p] = (pg[p] * Hkv + g) * 2;
-                    if (key0 + kSlotKeys < w.kv_end) load_pages(key0 + kSlotKeys);      // next tile's page ids in flight
-                    const uint32_t lt = (lastT >> (2 * s)) & 3u;
-                    const uint32_t epar = ((lt == 1 ? parP : parD) >> s) & 1u;
-                    if (lt) mbar_wait(BAR((lt == 1 ? B_VEMPTY_P : B_VEMPTY_D) + s), epar);
-                    mbar_arrive_expect_tx(BAR(B_VFULL + s), (uint32_t)npages * SM::kPageBytes);
-#pragma unroll
-                    for (int p = 0; p < 4; ++p)
-                        if (p < npages) tma_load_slab(sbase + SM::kVOff + s * SM::kSlot + p * SM::kPageBytes, &tmap_v, cgrp[p], BAR(B_VFULL + s));
-                    if (lt == 1) parP ^= 1u << s; else if (lt == 2) parD ^= 1u << s;
-                    lastT = (lastT & ~(3u << (2 * s))) | ((uint32_t)w.kind << (2 * s));
-                }
+                for (int p = 0; p < 4; ++p) pg[p] = (w.kv_begin + p * kPage < w.kv_end) ? __ldg(bt + (w.kv_begin >> 4) + p) : 0;
+                vs.item(w, bt, g, Hkv, pg, []() {});
                 mbar_arrive(BAR(B_SCHED_EMPTY + slot));
             }
         }
