@@ -38,9 +38,10 @@
 #include "plan.cuh"
 #include "ptx.cuh"
 
-// -DSS_PROFILE (measurement builds only, see profiles/): clock64 phase counters of the prefill loop, written into the
-// ss_debug_set_trace buffer - per item words 5..8 = chain A's cycles in {S wait, tcgen05.ld, softmax, st + fence +
-// arrive}; the last 4 words of the CTA block = the MMA thread's cycles in {P wait, K/V wait, issue} and its half tiles.
+// -DSS_PROFILE (measurement builds only, see profiles/): clock64 phase counters, written into the ss_debug_set_trace
+// buffer - prefill items: words 5..8 = chain A's cycles in {S wait, tcgen05.ld, softmax, st + fence + arrive}, and the
+// last 4 words of the CTA block = the MMA thread's cycles in {P wait, K/V wait, issue} and its half tiles; decode items:
+// words 7, 8 = decode warp 0's cycles in {K wait << 32 | S^T, V wait << 32 | softmax + O^T} summed over the item's tiles.
 #ifdef SS_PROFILE
 #define SS_PF(i) { const long long c_ = clock64(); pf_acc[i] += c_ - pf_t; pf_t = c_; }
 #define SS_MM(i) { const long long c_ = clock64(); mm_acc[i] += c_ - mm_t; mm_t = c_; }
@@ -55,10 +56,7 @@ using namespace ptx;
 
 constexpr int kMixThreads = 384;
 constexpr int kSlotKeys = 64;        // keys per K / V ring slot = keys per S buffer
-#ifndef SS_NUM_ST
-#define SS_NUM_ST 5
-#endif
-constexpr int kNumSt = SS_NUM_ST;    // K ring slots = V ring slots
+constexpr int kNumSt = 5;            // K ring slots = V ring slots (4: -1.5 % on pure decode, 6 would not leave room for 2 Q tiles)
 constexpr int kSchedSlots = 4;
 constexpr int kDecKeys = 16;         // keys of a 64-key slot one decode warp owns (4 warps per slot)
 // setmaxnreg moves registers inside the CTA's own launch allocation: 384 threads x 168 (the __launch_bounds__ cap ptxas
@@ -87,13 +85,7 @@ struct MixSmem {
     static constexpr int kKOff = 0;
     static constexpr int kVOff = kKOff + kNumSt * kSlot;
     static constexpr int kQOff = kVOff + kNumSt * kSlot;         // 2 Q tiles (prefill) / decode: cross-warp merge buffer + staged Q rows
-#ifndef SS_Q_TILES
-#define SS_Q_TILES 2
-#endif
-#ifndef SS_Q_EXTRA
-#define SS_Q_EXTRA 0
-#endif
-    static constexpr int kQBytes = SS_Q_TILES * kQTile + SS_Q_EXTRA;
+    static constexpr int kQBytes = 2 * kQTile;
     static constexpr int kMergeBytes = 4 * kMaxGroup * (D + 2) * 4;
     // decode with G <= 8: merge buffer of 8 rows per warp, then kSchedSlots staged Q blocks (G rows x D bf16, one per
     // scheduler slot, bulk-copied by the producer so the workers never wait on a cold global Q load)
@@ -261,6 +253,9 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
     // than one phase away from the barrier, and with 5 ring slots a slot alternates between the two warpgroups.
     const int r16 = cw * kDecKeys;                          // first key row of this warp inside its slots
     const int mi = lane >> 3, l7 = lane & 7;                // ldmatrix: this lane addresses row l7 of matrix mi
+#ifdef SS_PROFILE
+    long long pf_t = clock64(), pf_acc[4] = {0, 0, 0, 0};     // K wait | S^T | V wait | softmax + O^T  (cycles, this warp)
+#endif
     for (int t = 0; t < n; ++t) {
         const uint32_t tc = tile_ctr + t;
         const int s = tc % kNumSt;
@@ -272,6 +267,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
         float sT[NT][4];
         mbar_wait(BAR(B_KFULL + s), fpar);
         if (tr && t == 0) tr[3] = globaltimer_ns();
+        SS_PF(0)
         if (nvalid > 0) {
             // S^T (16 keys x 8 heads) = K (16 x D) Q^T: two interleaved accumulation chains per head tile
             float sU[NT][4];
@@ -295,7 +291,9 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(BAR(B_KEMPTY_D + s));
+        SS_PF(1)
         mbar_wait(BAR(B_VFULL + s), fpar);
+        SS_PF(2)
         if (nvalid > 0) {
             if (nvalid < kDecKeys) {
                 // zero the V rows past the end of the KV range (unused slots may hold NaN; 0 * NaN = NaN)
@@ -360,7 +358,11 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(BAR(B_VEMPTY_D + s));
+        SS_PF(3)
     }
+#ifdef SS_PROFILE
+    if (tr) { tr[7] = ((unsigned long long)pf_acc[0] << 32) | (unsigned)pf_acc[1]; tr[8] = ((unsigned long long)pf_acc[2] << 32) | (unsigned)pf_acc[3]; }
+#endif
     // ---- cross-warp log-sum-exp merge through smem, two stages over one 4-warp buffer [warp][head][D + 2] ----
     if (tr) tr[4] = globaltimer_ns();
 #pragma unroll
