@@ -16,7 +16,8 @@
  *     says so.
  *   - Return value: 0 = SS_OK, negative = error (see ss_status).  No exceptions, no abort().
  *   - Layouts (the paper is silent on them):
- *       k_cache, v_cache : [num_pages][num_kv_heads][page_size][head_dim] bf16   (4 KB slab per page,head)
+ *       k_cache, v_cache : [num_pages][num_kv_heads][page_size][head_dim] bf16   (4 KB slab per page,head;
+ *                          one byte per element with SS_FLAG_KV_FP8)
  *       block_table      : [R][max_pages_per_req] int32; entry p of row r is the physical page holding
  *                          logical tokens 16p..16p+15 of request r; entries past ceil((u_r+c_r)/16)
  *                          are never read
@@ -64,6 +65,7 @@ typedef enum ss_status {
 
 /* ss_config.flags */
 #define SS_FLAG_DEBUG_CHECKS 1u      /* "debug build" of SURVEY.md section 8(b): bounds-check device metadata in-kernel */
+#define SS_FLAG_KV_FP8 2u            /* FP8 E4M3 KV cache (reading 23): see ss_set_kv_scales */
 
 typedef struct ss_handle ss_handle;  /* opaque; owns tensor maps, SM count, small staging buffers */
 
@@ -76,13 +78,30 @@ typedef struct ss_config {
     int32_t max_requests;       /* upper bound on R */
     int32_t max_tokens;         /* upper bound on T */
     int32_t max_pages_per_req;  /* second dimension of block_table */
-    uint32_t flags;             /* 0 or SS_FLAG_DEBUG_CHECKS */
+    uint32_t flags;             /* bitwise or of SS_FLAG_* (0 = bf16 cache, no device checks) */
 } ss_config;
 
 /* Lifetime.  ss_create binds the handle to the two cache tensors (TMA descriptors are encoded once)
  * and to the current CUDA device.  The caches stay caller-owned and must outlive the handle. */
 int ss_create(ss_handle** out_handle, const ss_config* cfg, void* k_cache_device, void* v_cache_device);
 int ss_destroy(ss_handle* h);
+
+/*
+ * FP8 KV cache (SS_FLAG_KV_FP8; head_dim must be 128).  k_cache / v_cache are [num_pages][num_kv_heads][16][head_dim]
+ * bytes holding OCP FP8 E4M3 codes ("e4m3fn": bias 7, no infinities, max 448, S.1111.111 = NaN) with one fp32 scale per
+ * (tensor, kv head): value = decode(code) * scale[g].  k_scale_device / v_scale_device are DEVICE arrays of
+ * num_kv_heads floats, caller-owned, read by every later hot call (they must stay valid and may be rewritten between
+ * calls in stream order); every scale must be finite and > 0.  Required before the first ss_kv_append /
+ * ss_mixed_attention on an FP8 handle (SS_ERR_INVALID_ARG otherwise).
+ *   ss_kv_append       quantises: code = e4m3(x / scale[g]), the quotient an IEEE fp32 division, rounded to nearest
+ *                      even, magnitudes above 448 saturate to 448, NaN -> 0x7F.  Bit-exact against that definition.
+ *   ss_mixed_attention same definition as the bf16 path with K = decode(code) * k_scale[g], V likewise; bf16 q / out.
+ *                      Decode requests (c_r == 1) run on the split-KV tensor-core path over the FP8 tiles (half the HBM
+ *                      bytes; q is rounded to fp16 for the products: exact for |q| in [2^-14, 65504], clamped above);
+ *                      prefill chunks (c_r > 1) are served by the plain CUDA-core kernel in this version (correct, slow).
+ *   ss_qkv_rope_append returns SS_ERR_NOT_IMPLEMENTED on an FP8 handle.
+ */
+int ss_set_kv_scales(ss_handle* h, const float* k_scale_device, const float* v_scale_device);
 
 /* Upper bound (from the config) of the device workspace ss_mixed_attention needs: work list,
  * counters and split-KV partials. */

@@ -18,9 +18,11 @@ SS_OK = 0
 SS_ERR_INVALID_ARG = -1
 SS_ERR_DEVICE_CHECK = -6
 SS_FLAG_DEBUG_CHECKS = 1
+SS_FLAG_KV_FP8 = 2
 # include/slidingattn.h (the product boundary) ...
 EXPORTS = ["ss_version", "ss_status_string", "ss_last_error_string", "ss_create", "ss_destroy",
-           "ss_workspace_bytes", "ss_kv_append", "ss_qkv_rope_append", "ss_mixed_attention", "ss_iteration_host",
+           "ss_workspace_bytes", "ss_set_kv_scales", "ss_kv_append", "ss_qkv_rope_append", "ss_mixed_attention",
+           "ss_iteration_host",
            "ss_poll_device_error", "ss_reset"]
 # ... and include/slidingattn_debug.h (test / tuning / measurement aids)
 DEBUG_EXPORTS = ["ss_build_worklist", "ss_last_launch_count", "ss_debug_force_simple_path",
@@ -67,6 +69,7 @@ def load():
     lib.ss_destroy.argtypes = [vp]
     lib.ss_workspace_bytes.argtypes = [vp]
     lib.ss_workspace_bytes.restype = ctypes.c_size_t
+    lib.ss_set_kv_scales.argtypes = [vp, vp, vp]
     lib.ss_kv_append.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, vp]
     lib.ss_qkv_rope_append.argtypes = [vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
     lib.ss_mixed_attention.argtypes = [vp, vp, vp, vp, vp, i32, i32, f32, vp, vp, vp, ctypes.c_size_t, vp]
@@ -114,25 +117,38 @@ def _stream_ptr(stream) -> Optional[int]:
 
 
 class SlidingAttn:
-    """Handle bound to one pair of paged caches [num_pages, Hkv, 16, D] bf16 on the current device."""
+    """Handle bound to one pair of paged caches [num_pages, Hkv, 16, D] on the current device: bf16, or uint8 E4M3
+    codes (SS_FLAG_KV_FP8; then `kv_scales` = (k_scale, v_scale), float32 CUDA tensors of Hkv entries each)."""
 
     def __init__(self, num_q_heads: int, num_kv_heads: int, head_dim: int, k_cache: torch.Tensor,
                  v_cache: torch.Tensor, max_requests: int, max_tokens: int, max_pages_per_req: int,
-                 debug_checks: bool = False):
+                 debug_checks: bool = False, kv_scales=None):
         self.lib = load()
         if not (k_cache.is_cuda and v_cache.is_cuda):
             raise SlidingAttnError("caches must be CUDA tensors (no CPU path exists)")
-        assert k_cache.dtype == torch.bfloat16 and k_cache.is_contiguous() and k_cache.shape == v_cache.shape
+        fp8 = k_cache.dtype == torch.uint8
+        assert (fp8 or k_cache.dtype == torch.bfloat16) and v_cache.dtype == k_cache.dtype
+        assert k_cache.is_contiguous() and v_cache.is_contiguous() and k_cache.shape == v_cache.shape
         P, Hkv, page, D = k_cache.shape
         assert Hkv == num_kv_heads and D == head_dim
+        flags = (SS_FLAG_DEBUG_CHECKS if debug_checks else 0) | (SS_FLAG_KV_FP8 if fp8 else 0)
         self.cfg = ss_config(num_q_heads, num_kv_heads, head_dim, page, P, max_requests, max_tokens,
-                             max_pages_per_req, SS_FLAG_DEBUG_CHECKS if debug_checks else 0)
+                             max_pages_per_req, flags)
         self.k_cache, self.v_cache = k_cache, v_cache
         self._h = ctypes.c_void_p()
         self._check(self.lib.ss_create(ctypes.byref(self._h), ctypes.byref(self.cfg), k_cache.data_ptr(),
                                        v_cache.data_ptr()), create=True)
         self.workspace_bytes = int(self.lib.ss_workspace_bytes(self._h))
         self.workspace = torch.empty(self.workspace_bytes, dtype=torch.uint8, device=k_cache.device)
+        if kv_scales is not None:
+            self.set_kv_scales(*kv_scales)
+
+    def set_kv_scales(self, k_scale: torch.Tensor, v_scale: torch.Tensor):
+        """FP8 handles: per kv head fp32 scales (device tensors; the handle keeps them alive and the kernels read them)."""
+        _want(k_scale, "k_scale", torch.float32, True, (self.cfg.num_kv_heads,))
+        _want(v_scale, "v_scale", torch.float32, True, (self.cfg.num_kv_heads,))
+        self.k_scale, self.v_scale = k_scale, v_scale
+        self._check(self.lib.ss_set_kv_scales(self._h, k_scale.data_ptr(), v_scale.data_ptr()))
 
     def _check(self, rc: int, create: bool = False):
         if rc != SS_OK:
@@ -273,8 +289,9 @@ def mixed_attention(handle: SlidingAttn, q, block_table, query_start_loc, ctx_le
     return handle.mixed_attention(q, block_table, query_start_loc, ctx_lens, scale, out, lse, stream)
 
 
-def handle_for(batch, tensors, extra_tokens: int = 0, debug_checks: bool = False) -> SlidingAttn:
-    """Convenience: a handle sized for one workloads.Batch."""
-    return SlidingAttn(batch.num_q_heads, batch.num_kv_heads, batch.head_dim, tensors.k_cache, tensors.v_cache,
+def handle_for(batch, tensors, extra_tokens: int = 0, debug_checks: bool = False, fp8_caches=None, kv_scales=None) -> SlidingAttn:
+    """Convenience: a handle sized for one workloads.Batch (fp8_caches = (k_codes, v_codes) uint8 tensors for an FP8 handle)."""
+    kc, vc = fp8_caches if fp8_caches is not None else (tensors.k_cache, tensors.v_cache)
+    return SlidingAttn(batch.num_q_heads, batch.num_kv_heads, batch.head_dim, kc, vc,
                        max_requests=max(batch.R, 1), max_tokens=max(batch.T + extra_tokens, 1),
-                       max_pages_per_req=batch.max_pages_per_req, debug_checks=debug_checks)
+                       max_pages_per_req=batch.max_pages_per_req, debug_checks=debug_checks, kv_scales=kv_scales)

@@ -52,9 +52,11 @@ int encode_cache_map(Handle* h, CUtensorMap* map, void* base) {
         return SS_ERR_CUDA;
     }
     const ss_config& c = h->cfg;
-    const cuuint32_t halves = (cuuint32_t)c.head_dim / 64;
+    // FP8 cache: a row is head_dim bytes; the same map in units of 2-byte words (64 words = 128 bytes per half row)
+    const cuuint64_t row_bytes = (cuuint64_t)c.head_dim * (h->kv_fp8 ? 1 : 2);
+    const cuuint32_t halves = (cuuint32_t)(row_bytes / 128);
     cuuint64_t gdim[4] = {64, 8, halves, (cuuint64_t)c.num_pages * c.num_kv_heads * 2};
-    cuuint64_t gstride[3] = {(cuuint64_t)c.head_dim * 2, 128, (cuuint64_t)c.head_dim * 2 * 8};
+    cuuint64_t gstride[3] = {row_bytes, 128, row_bytes * 8};
     cuuint32_t box[4] = {64u, 8u, halves, 2u};
     cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
     CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, base, gdim, gstride, box, estr,
@@ -113,7 +115,8 @@ int ss_create(ss_handle** out_handle, const ss_config* cfg, void* k_cache, void*
         cfg->max_pages_per_req <= 0)
         return SS_ERR_INVALID_ARG;
     if ((int64_t)cfg->max_pages_per_req * kPage > (int64_t)1 << 30) return SS_ERR_INVALID_ARG;
-    if (cfg->flags & ~(uint32_t)SS_FLAG_DEBUG_CHECKS) return SS_ERR_INVALID_ARG;
+    if (cfg->flags & ~(uint32_t)(SS_FLAG_DEBUG_CHECKS | SS_FLAG_KV_FP8)) return SS_ERR_INVALID_ARG;
+    if ((cfg->flags & SS_FLAG_KV_FP8) && cfg->head_dim != 128) return SS_ERR_INVALID_ARG;
     if (!workspace_layout(*cfg, 256).ok) return SS_ERR_INVALID_ARG;   // worst-case item count must fit the int32 index space
 
     int dev = 0;
@@ -132,12 +135,13 @@ int ss_create(ss_handle** out_handle, const ss_config* cfg, void* k_cache, void*
     h->k_cache = k_cache;
     h->v_cache = v_cache;
     h->debug_checks = (cfg->flags & SS_FLAG_DEBUG_CHECKS) ? 1 : 0;
+    h->kv_fp8 = (cfg->flags & SS_FLAG_KV_FP8) ? 1 : 0;
     h->ws = workspace_layout(h->cfg, h->num_sms);
     if (!h->ws.ok) {                 // worst-case item count of this config overflows the int32 index space
         delete h;
         return SS_ERR_INVALID_ARG;
     }
-    if (init_main_attention(cfg->head_dim) != cudaSuccess) {
+    if (init_main_attention(cfg->head_dim, h->kv_fp8) != cudaSuccess) {
         delete h;
         return SS_ERR_CUDA;
     }
@@ -169,6 +173,14 @@ int ss_destroy(ss_handle* hh) {
     for (void* b : bufs)
         if (b) cudaFree(b);
     delete h;
+    return SS_OK;
+}
+
+int ss_set_kv_scales(ss_handle* hh, const float* k_scale, const float* v_scale) {
+    Handle* h = (Handle*)hh;
+    if (!h || !h->kv_fp8 || !k_scale || !v_scale || (((uintptr_t)k_scale) & 3u) || (((uintptr_t)v_scale) & 3u)) return SS_ERR_INVALID_ARG;
+    h->k_scale = k_scale;
+    h->v_scale = v_scale;
     return SS_OK;
 }
 
@@ -240,6 +252,7 @@ int ss_kv_append(ss_handle* hh, const void* k_new, const void* v_new, const int3
     h->last_launches = 0;
     if (R == 0 || T == 0) return SS_OK;
     if (!block_table || (((uintptr_t)block_table) & 3u)) return SS_ERR_INVALID_ARG;
+    if (h->kv_fp8 && !h->k_scale) return SS_ERR_INVALID_ARG;          // ss_set_kv_scales first
     if (h->debug_checks)
         SS_CUDA(h, launch_validate(h, block_table, query_start_loc, ctx_lens, R, T, (cudaStream_t)cuda_stream), "validate launch");
     SS_CUDA(h, launch_kv_append(h, k_new, v_new, block_table, query_start_loc, ctx_lens, R, T, (cudaStream_t)cuda_stream),
@@ -257,6 +270,7 @@ int ss_qkv_rope_append(ss_handle* hh, const void* qkv, const int32_t* block_tabl
     if (R == 0 || T == 0) return SS_OK;
     if (!block_table || (((uintptr_t)block_table) & 3u)) return SS_ERR_INVALID_ARG;
     if (!(rope_theta > 1.f) || !isfinite(rope_theta)) return SS_ERR_INVALID_ARG;
+    if (h->kv_fp8) return SS_ERR_NOT_IMPLEMENTED;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (h->debug_checks) SS_CUDA(h, launch_validate(h, block_table, query_start_loc, ctx_lens, R, T, st), "validate launch");
     SS_CUDA(h, launch_qkv_rope_append(h, qkv, block_table, query_start_loc, ctx_lens, R, T, rope_theta, q_out, st),
@@ -278,6 +292,7 @@ int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table,
     if (!workspace || !aligned16(workspace)) return SS_ERR_INVALID_ARG;
     if (workspace_bytes < h->ws.total) return SS_ERR_WORKSPACE_TOO_SMALL;
     if (!(scale > 0.f) || !isfinite(scale)) return SS_ERR_INVALID_ARG;      // see slidingattn.h: running max of raw scores
+    if (h->kv_fp8 && !h->k_scale) return SS_ERR_INVALID_ARG;                // ss_set_kv_scales first
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (h->debug_checks) SS_CUDA(h, launch_validate(h, block_table, query_start_loc, ctx_lens, R, T, st), "validate launch");
 
@@ -297,6 +312,12 @@ int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table,
     if (h->timing_on) {
         SS_CUDA(h, cudaEventRecord(h->ev1, st), "timing event");
         h->timing_valid = 1;
+    }
+    if (h->kv_fp8) {
+        // prefill chunks over an FP8 cache: the plain CUDA-core kernel (the main kernel's plan skipped them)
+        SS_CUDA(h, launch_simple_attention(h, q, block_table, query_start_loc, ctx_lens, R, T, scale, out, lse_or_null, st, 1),
+                "simple attention launch (FP8 prefill rows)");
+        ++n;
     }
     h->last_launches = (two_kernels ? 1 : 0) + n + h->debug_checks;
     return SS_OK;

@@ -68,16 +68,19 @@ constexpr float kMLog2e = 1.4426950408889634f;
 constexpr float kMLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.f;   // log2 units: P <= 2^8, safe in bf16 / fp32
 
-template <int D>
+// FP8: the KV cache holds one byte per element (E4M3 codes): a key row is D bytes = D/128 128-byte chunks; the ring
+// keeps the bf16 slot size (half of each slot stays unused) so every other offset is the same in both instantiations.
+template <int D, bool FP8 = false>
 struct MixSmem {
-    static constexpr int kHalves = D / 64;
+    static constexpr int kHalves = D / 64;                       // 128-byte chunks of a bf16 row (Q tiles, bf16 K / V rows)
+    static constexpr int kKvHalves = FP8 ? D / 128 : D / 64;     // 128-byte chunks of a K / V row in the ring
     static constexpr int kSlot = kHalves * kSlotKeys * 128;      // one K (or V) ring slot
     // Slot layout = what ONE 4-D TMA box per (page, kv head) slab writes: [8-key group][64-column half][8 rows][128 B],
     // every [8 rows][128 B] block a SWIZZLE_128B core group.  8-key groups are kGroup bytes apart (uniform over the 4
     // pages of a slot: the UMMA stride-byte-offset), the halves of a group 1024 bytes apart.
-    static constexpr int kGroup = kHalves * 1024;
+    static constexpr int kGroup = kKvHalves * 1024;
     static constexpr int kPageBytes = 2 * kGroup;                // one (page, kv head) slab: 16 keys
-    // byte offset of the 16-byte chunk cd (0 .. D/8-1) of key row r (0 .. 63) inside a slot, swizzle applied
+    // byte offset of the 16-byte chunk cd (0 .. 8 kKvHalves - 1) of key row r (0 .. 63) inside a slot, swizzle applied
     __device__ static __forceinline__ uint32_t kv_off(int r, int cd) {
         return (uint32_t)((r >> 3) * kGroup + (cd >> 3) * 1024 + (r & 7) * 128 + (((cd & 7) ^ (r & 7)) << 4));
     }
@@ -150,6 +153,8 @@ struct MixParams {
     int self_plan, R, num_sms, force_split_keys, force_decode_ctas;
     unsigned long long* trace;     // ss_debug_set_trace: per-CTA timeline, or null
     int trace_words;
+    const float* k_scale;          // SS_FLAG_KV_FP8: per kv head scales (device), else null
+    const float* v_scale;
     const int32_t* err_flag;       // SS_FLAG_DEBUG_CHECKS: nonzero = the metadata check tripped, serve no item; else null
 };
 
@@ -207,26 +212,45 @@ __device__ __forceinline__ float softmax_half(uint32_t (&sr)[2][32], int nvis, f
     return alpha;
 }
 
+// bf16 pair -> fp16 pair (FP8 cache: the products run as f16 MMAs, every E4M3 value being an fp16 value).  Exact for
+// magnitudes in [2^-14, 65504]; clamped above (documented in slidingattn.h), rounded to the fp16 subnormal grid below.
+__device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t w) {
+    const float lo = fminf(fmaxf(__uint_as_float(w << 16), -65504.f), 65504.f);
+    const float hi = fminf(fmaxf(__uint_as_float(w & 0xffff0000u), -65504.f), 65504.f);
+    return pack_f16(lo, hi);
+}
+
 // One decode split on the 8 worker warps (see the call site).  NT = 8-head column tiles (1: G <= 8, 2: G <= 16).
-template <int D, int NT>
+// FP8 (E4M3 cache, reading 23): the same structure on 128-byte key rows.  ldmatrix moves the codes as 16-bit
+// units, so a thread ends up with 4 consecutive d of one key (K) or a 2 x 2 block of (key, d) (V, transposed load):
+//   S^T: the contraction index is permuted inside each 16-d step - MMA k = {2c, 2c+1, 2c+8, 2c+9} <-> d = 16 ks + {4c,
+//        4c+1, 4c+2, 4c+3} - identically for the K fragment and the Q^T fragment (a sum does not care);
+//   O^T: one byte permute per register separates the two d of a block; MMA row i < 8 <-> d = 16 mt + 2i, row i + 8 <->
+//        d = 16 mt + 2i + 1, undone when the accumulators are written out.
+// Codes widen exactly to fp16 (cvt.rn.f16x2.e4m3x2), P is rounded to fp16, k_scale folds into the score scale and
+// v_scale into the output.
+template <int D, int NT, bool FP8>
 __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, const int slot, const uint32_t tile_ctr,
                                             const int wg, const int cw, const int lane, const int wtid, const uint32_t sbase,
                                             const uint32_t bar0, const MixParams& prm, float* merge, unsigned long long* tr) {
-    using SM = MixSmem<D>;
-    constexpr int kHalves = SM::kHalves;
+    using SM = MixSmem<D, FP8>;
+    constexpr int kHalves = SM::kKvHalves;
     auto BAR = [&](int i) -> uint32_t { return bar0 + 8u * (uint32_t)i; };
     const int Hq = prm.Hq, Hkv = prm.Hkv, G = Hq / Hkv;
-    const float sl2 = prm.scale * kMLog2e;
+    const float sl2 = prm.scale * kMLog2e * (FP8 ? __ldg(prm.k_scale + w.head) : 1.f);
+    const float vs = FP8 ? __ldg(prm.v_scale + w.head) : 1.f;
     const int qr = lane >> 2, qc = (lane & 3) * 2;           // fragment coordinates: row / column pair
     constexpr int mrows = NT * 8;                           // merge-buffer rows (heads) per warp
-    // B fragments of Q^T (16 d x 8 heads per k-step): head = 8 nt + qr, d = 16 ks + qc (+1) and + 8
+    // B fragments of Q^T (16 d x 8 heads per k-step): head = 8 nt + qr; bf16: d = 16 ks + qc (+1) and + 8;
+    // FP8: d = 16 ks + 2 qc (+1) and + 2 (+3), as fp16 pairs
     uint32_t qb[D / 16][2 * NT];
     if (NT == 1) {
-        const uint32_t qs = sbase + SM::kQStageOff + slot * SM::kQStageBytes + (qr * D + qc) * 2;
+        const uint32_t qs = sbase + SM::kQStageOff + slot * SM::kQStageBytes + (qr * D + (FP8 ? 2 : 1) * qc) * 2;
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks) {
-            qb[ks][0] = qr < G ? lds32(qs + ks * 32) : 0u;
-            qb[ks][1] = qr < G ? lds32(qs + ks * 32 + 16) : 0u;
+            const uint32_t w0 = qr < G ? lds32(qs + ks * 32) : 0u, w1 = qr < G ? lds32(qs + ks * 32 + (FP8 ? 4 : 16)) : 0u;
+            qb[ks][0] = FP8 ? bf16x2_to_f16x2(w0) : w0;
+            qb[ks][1] = FP8 ? bf16x2_to_f16x2(w1) : w1;
         }
     } else {
         const __nv_bfloat16* qg = prm.q + ((int64_t)w.row0 * Hq + (int64_t)w.head * G) * D;
@@ -235,11 +259,15 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
 #pragma unroll
             for (int ks = 0; ks < D / 16; ++ks) {
                 const int hd = 8 * nt + qr;
-                qb[ks][2 * nt] = hd < G ? *reinterpret_cast<const uint32_t*>(qg + (int64_t)hd * D + ks * 16 + qc) : 0u;
-                qb[ks][2 * nt + 1] = hd < G ? *reinterpret_cast<const uint32_t*>(qg + (int64_t)hd * D + ks * 16 + qc + 8) : 0u;
+                const __nv_bfloat16* src = qg + (int64_t)hd * D + ks * 16 + (FP8 ? 2 : 1) * qc;
+                const uint32_t w0 = hd < G ? *reinterpret_cast<const uint32_t*>(src) : 0u;
+                const uint32_t w1 = hd < G ? *reinterpret_cast<const uint32_t*>(src + (FP8 ? 2 : 8)) : 0u;
+                qb[ks][2 * nt] = FP8 ? bf16x2_to_f16x2(w0) : w0;
+                qb[ks][2 * nt + 1] = FP8 ? bf16x2_to_f16x2(w1) : w1;
             }
     }
     // O^T accumulators: [nt][mt] c0 = (d = 16 mt + qr, head 8 nt + qc), c1 = head + 1, c2 = (d + 8, head), c3 = (d + 8, head + 1)
+    // (FP8: c0 / c1 at d = 16 mt + 2 qr, c2 / c3 at d + 1)
     float oT[NT][D / 16][4];
     float m[NT][2], l[NT][2];                               // per head qc, qc + 1 (l: this lane's share of the row sum)
 #pragma unroll
@@ -276,6 +304,22 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
 #pragma unroll
                 for (int i = 0; i < 4; ++i) sT[nt][i] = sU[nt][i] = 0.f;
             const int rk = r16 + (mi & 1) * 8 + l7;          // a0: keys 0-7, a1: keys 8-15, a2 / a3: the next 8 d
+            if (FP8) {
+#pragma unroll
+                for (int jj = 0; jj < D / 32; ++jj) {            // one ldmatrix = 16 keys x 32 d of codes = two k-steps
+                    const int cd = 2 * jj + (mi >> 1);
+                    uint32_t r[4];
+                    ldmatrix_x4(r[0], r[1], r[2], r[3], kbase + SM::kv_off(rk, cd));
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const int ks = 2 * jj + h;
+                        const uint32_t a[4] = {e4m3x2_to_f16x2(r[2 * h]), e4m3x2_to_f16x2(r[2 * h + 1]),
+                                               e4m3x2_hi_to_f16x2(r[2 * h]), e4m3x2_hi_to_f16x2(r[2 * h + 1])};
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt) mma_f16_16816(h ? sU[nt] : sT[nt], a, qb[ks][2 * nt], qb[ks][2 * nt + 1]);
+                    }
+                }
+            } else {
 #pragma unroll
             for (int ks = 0; ks < D / 16; ++ks) {
                 const int cd = 2 * ks + (mi >> 1);
@@ -283,6 +327,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
                 ldmatrix_x4(a[0], a[1], a[2], a[3], kbase + SM::kv_off(rk, cd));
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) mma_bf16_16816((ks & 1) ? sU[nt] : sT[nt], a, qb[ks][2 * nt], qb[ks][2 * nt + 1]);
+            }
             }
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt)
@@ -326,8 +371,8 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
                 const float p2 = exp2f(sT[nt][2] * sl2 - mn[nt][0]), p3 = exp2f(sT[nt][3] * sl2 - mn[nt][1]);
                 sT[nt][0] = p0 + p2;                         // this lane's share of the two row sums
                 sT[nt][1] = p1 + p3;
-                pb[nt][0] = movmatrix_trans(pack_bf16(p0, p1));   // keys 0-7:  (key qr, heads qc..) -> (head qr, keys qc..)
-                pb[nt][1] = movmatrix_trans(pack_bf16(p2, p3));   // keys 8-15
+                pb[nt][0] = movmatrix_trans(FP8 ? pack_f16(p0, p1) : pack_bf16(p0, p1));   // keys 0-7:  (key qr, heads qc..) -> (head qr, keys qc..)
+                pb[nt][1] = movmatrix_trans(FP8 ? pack_f16(p2, p3) : pack_bf16(p2, p3));   // keys 8-15
             }
             // the accumulators are only rescaled when some head's maximum moved (warp-uniform test)
             if (__any_sync(0xffffffffu, moved)) {
@@ -345,6 +390,23 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt) { l[nt][0] += sT[nt][0]; l[nt][1] += sT[nt][1]; }
             // O^T (D x 8 heads) += V^T (D x 16 keys) P^T: a0 = (keys 0-7, d 0-7)^T, a1 = (keys 0-7, d 8-15)^T, a2 / a3: keys 8-15
+            if (FP8) {
+                const int rv = r16 + (mi & 1) * 8 + l7;          // matrices: (keys 0-7, chunk), (keys 8-15, chunk), the same for chunk + 1
+#pragma unroll
+                for (int mm = 0; mm < D / 32; ++mm) {
+                    const int cd = 2 * mm + (mi >> 1);
+                    uint32_t r[4];
+                    ldmatrix_x4_trans(r[0], r[1], r[2], r[3], vbase + SM::kv_off(rv, cd));
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        // register = codes [key 2c][d 2qr], [2c][2qr+1], [2c+1][2qr], [2c+1][2qr+1] -> (d 2qr | d 2qr+1) x keys (2c, 2c+1)
+                        const uint32_t x0 = __byte_perm(r[2 * h], 0u, 0x3120), x1 = __byte_perm(r[2 * h + 1], 0u, 0x3120);
+                        const uint32_t a[4] = {e4m3x2_to_f16x2(x0), e4m3x2_hi_to_f16x2(x0), e4m3x2_to_f16x2(x1), e4m3x2_hi_to_f16x2(x1)};
+#pragma unroll
+                        for (int nt = 0; nt < NT; ++nt) mma_f16_16816(oT[nt][2 * mm + h], a, pb[nt][0], pb[nt][1]);
+                    }
+                }
+            } else {
             const int rv = r16 + (mi >> 1) * 8 + l7;
 #pragma unroll
             for (int mt = 0; mt < D / 16; ++mt) {
@@ -353,6 +415,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
                 ldmatrix_x4_trans(a[0], a[1], a[2], a[3], vbase + SM::kv_off(rv, cd));
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) mma_bf16_16816(oT[nt][mt], a, pb[nt][0], pb[nt][1]);
+            }
             }
             if (nvalid < kDecKeys) fence_proxy_async();
         }
@@ -373,6 +436,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
             l[nt][1] += __shfl_xor_sync(0xffffffffu, l[nt][1], o);
         }
     float* mine = merge + cw * mrows * (D + 2);
+    const int dA = FP8 ? 2 * qr : qr, dB = FP8 ? 2 * qr + 1 : qr + 8;     // d (inside a 16-d block) of accumulator rows qr, qr + 8
     auto put = [&]() {
 #pragma unroll
         for (int nt = 0; nt < NT; ++nt) {
@@ -380,10 +444,10 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
             float* h1 = h0 + (D + 2);
 #pragma unroll
             for (int mt = 0; mt < D / 16; ++mt) {
-                h0[16 * mt + qr] = oT[nt][mt][0];
-                h1[16 * mt + qr] = oT[nt][mt][1];
-                h0[16 * mt + qr + 8] = oT[nt][mt][2];
-                h1[16 * mt + qr + 8] = oT[nt][mt][3];
+                h0[16 * mt + dA] = oT[nt][mt][0];
+                h1[16 * mt + dA] = oT[nt][mt][1];
+                h0[16 * mt + dB] = oT[nt][mt][2];
+                h1[16 * mt + dB] = oT[nt][mt][3];
             }
             if (qr == 0) {
                 h0[D] = m[nt][0]; h0[D + 1] = l[nt][0];
@@ -411,10 +475,10 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
         const float wa1 = m[nt][1] == -INFINITY ? 0.f : exp2f(m[nt][1] - M1), wb1 = mb1 == -INFINITY ? 0.f : exp2f(mb1 - M1);
 #pragma unroll
         for (int mt = 0; mt < D / 16; ++mt) {
-            oT[nt][mt][0] = oT[nt][mt][0] * wa0 + h0[16 * mt + qr] * wb0;
-            oT[nt][mt][1] = oT[nt][mt][1] * wa1 + h1[16 * mt + qr] * wb1;
-            oT[nt][mt][2] = oT[nt][mt][2] * wa0 + h0[16 * mt + qr + 8] * wb0;
-            oT[nt][mt][3] = oT[nt][mt][3] * wa1 + h1[16 * mt + qr + 8] * wb1;
+            oT[nt][mt][0] = oT[nt][mt][0] * wa0 + h0[16 * mt + dA] * wb0;
+            oT[nt][mt][1] = oT[nt][mt][1] * wa1 + h1[16 * mt + dA] * wb1;
+            oT[nt][mt][2] = oT[nt][mt][2] * wa0 + h0[16 * mt + dB] * wb0;
+            oT[nt][mt][3] = oT[nt][mt][3] * wa1 + h1[16 * mt + dB] * wb1;
         }
         l[nt][0] = l[nt][0] * wa0 + lb0 * wb0;
         l[nt][1] = l[nt][1] * wa1 + lb1 * wb1;
@@ -438,6 +502,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
             L += src[D + 1] * wgt;
             acc += src[d] * wgt;
         }
+        acc *= vs;
         if (w.nsplit == 1) {
             const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r;
             prm.out[orow * D + d] = __float2bfloat16_rn(acc / L);
@@ -464,9 +529,9 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
 // UTMALDG pairs can be scheduled together, and page ids are loaded two tiles ahead of their use.
 // Slot history as bit fields: parity of the next EMPTY wait per consumer type, and the type (1 prefill / 2 decode) of
 // the slot's last consumer, which names the EMPTY barrier that consumer will arrive on.
-template <int D, int B_FULL0, int B_EMPTY_P0, int B_EMPTY_D0>
+template <int D, bool FP8, int B_FULL0, int B_EMPTY_P0, int B_EMPTY_D0>
 struct TileStreamer {
-    using SM = MixSmem<D>;
+    using SM = MixSmem<D, FP8>;
     uint32_t parP = 0, parD = 0, lastT = 0;
     int s = 0;                     // ring slot of the next tile
     uint32_t eb = 0, epar = 0;     // EMPTY barrier (0: slot never used) and parity the next tile must see
@@ -589,11 +654,11 @@ __device__ __forceinline__ void split_merge(const ss_work_item& w, const int slo
     }
 }
 
-template <int D>
+template <int D, bool FP8>
 __global__ void __launch_bounds__(kMixThreads, 1)
 mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
              const __grid_constant__ CUtensorMap tmap_v, const MixParams prm) {
-    using SM = MixSmem<D>;
+    using SM = MixSmem<D, FP8>;
     constexpr int kHalves = SM::kHalves;
     extern __shared__ __align__(1024) uint8_t smem_raw[];       // SWIZZLE_128B tiles need 1024-byte alignment
     const uint32_t sbase = smem_u32(smem_raw);
@@ -658,7 +723,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     } else if (prm.self_plan) {
         // a2: every CTA builds the same plan (scratch = the still unused K ring); items are decoded from queue tickets
         build_plan<kMixThreads, uint16_t>(prm.qsl, prm.ctx_lens, prm.R, Hq, Hkv, D, prm.num_sms, prm.force_split_keys,
-                                          prm.force_decode_ctas, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph);
+                                          prm.force_decode_ctas, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph, FP8 ? 1 : 0);
         fence_proxy_async();    // scratch was written through the generic proxy; TMA writes the same bytes next
     } else if (threadIdx.x == 0) {
         ph->tot_p = prm.hdr->n_prefill;
@@ -683,7 +748,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             int32_t* const q_pre = prm.queue, * const q_dec = prm.queue + 1;
             bool pre_done = n_pre_items == 0, dec_done = n_dec == 0;
             // per-slot history as bit fields: parity of the next EMPTY wait per consumer type, last consumer type
-            TileStreamer<D, B_KFULL, B_KEMPTY_P, B_KEMPTY_D> ks;
+            TileStreamer<D, FP8, B_KFULL, B_KEMPTY_P, B_KEMPTY_D> ks;
             ks.bar0 = bar0; ks.ring = sbase + SM::kKOff; ks.tmap = &tmap_k;
             uint32_t n_sched = 0, n_pre = 0;
             int prev_kind = 0;
@@ -783,7 +848,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         // Follows the scheduler ring like every consumer and streams the V tiles of each item into the V ring: same slot
         // order and the same typed-EMPTY bookkeeping as warp 0 keeps for K.  One elected thread, waits included.
         if (elect_one()) {
-            TileStreamer<D, B_VFULL, B_VEMPTY_P, B_VEMPTY_D> vs;
+            TileStreamer<D, FP8, B_VFULL, B_VEMPTY_P, B_VEMPTY_D> vs;
             vs.bar0 = bar0; vs.ring = sbase + SM::kVOff; vs.tmap = &tmap_v;
             uint32_t n_sched = 0;
             for (;;) {
@@ -822,7 +887,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             const int n = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
             ++n_sched;
             if (kind == 0) break;
-            if (kind == 1) {
+            if (!FP8 && kind == 1) {
                 const int nq = w.nheads;
                 if (X < nq && elect_one()) {
                     const int ncommit = nq == 1 ? 2 : 1;          // arrivals this chain owes the shared (count 2) barriers
@@ -929,7 +994,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 tr[0] = globaltimer_ns();
                 tr[2] = ((unsigned long long)w.kind << 32) | (unsigned)n;
             }
-            if (w.kind == 1 && wg < w.nheads) {
+            if (!FP8 && w.kind == 1 && wg < w.nheads) {
                 // -------------------------- prefill tile, chain wg: thread = query row --------------------------
                 const int u = __ldg(prm.ctx_lens + w.req);
                 const int limit = u + w.q_pos0 + row + 1;            // keys [0, limit) visible to this row
@@ -1048,8 +1113,8 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 // movmatrix from the S^T accumulators).  With heads padded to M = 16 instead, a 64-key tile cost 128 HMMA
                 // and the legacy tensor path (~1 HMMA.16816 per 9 clk and SM) capped an SM at ~52 GB/s whatever the
                 // ring depth, copy mechanism or warp count (profiles/r2b.md); this form needs 64 (G <= 8).
-                if (G <= 8) decode_item<D, 1>(w, n, slot, tile_ctr, wg, cw, lane, wtid, sbase, bar0, prm, merge, tr);
-                else        decode_item<D, 2>(w, n, slot, tile_ctr, wg, cw, lane, wtid, sbase, bar0, prm, merge, tr);
+                if (G <= 8) decode_item<D, 1, FP8>(w, n, slot, tile_ctr, wg, cw, lane, wtid, sbase, bar0, prm, merge, tr);
+                else        decode_item<D, 2, FP8>(w, n, slot, tile_ctr, wg, cw, lane, wtid, sbase, bar0, prm, merge, tr);
             }
             tile_ctr += n;
             if (tr) tr[1] = globaltimer_ns();
@@ -1117,6 +1182,8 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     p.self_plan = main_self_plans(h, R, T) ? 1 : 0;
     p.merge_counters = p.self_plan ? h->state + kStateCounters : (int32_t*)(ws + h->ws.counters_off);
     p.err_flag = h->debug_checks ? h->state + kStateErr : nullptr;
+    p.k_scale = h->k_scale;
+    p.v_scale = h->v_scale;
     p.queue = p.self_plan ? h->state : &p.hdr->next_prefill;
     p.qsl = qsl;
     p.R = R;
@@ -1136,19 +1203,23 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     *n_launches = 1;
     const int grid = h->dbg[kDbgGrid] > 0 ? h->dbg[kDbgGrid] : h->num_sms;
     cudaError_t e;
-    if (c.head_dim == 128)
-        e = launch_pdl(mixed_kernel<128>, dim3(grid), dim3(kMixThreads), MixSmem<128>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+    if (h->kv_fp8)
+        e = launch_pdl(mixed_kernel<128, true>, dim3(grid), dim3(kMixThreads), MixSmem<128, true>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+    else if (c.head_dim == 128)
+        e = launch_pdl(mixed_kernel<128, false>, dim3(grid), dim3(kMixThreads), MixSmem<128>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
     else
-        e = launch_pdl(mixed_kernel<64>, dim3(grid), dim3(kMixThreads), MixSmem<64>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+        e = launch_pdl(mixed_kernel<64, false>, dim3(grid), dim3(kMixThreads), MixSmem<64>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
     if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 
 // Opt in to the large dynamic shared-memory window once per process and head_dim (ss_create), not per call.
-cudaError_t init_main_attention(int head_dim) {
+cudaError_t init_main_attention(int head_dim, int kv_fp8) {
+    if (kv_fp8)
+        return cudaFuncSetAttribute(mixed_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, MixSmem<128, true>::kTotal);
     if (head_dim == 128)
-        return cudaFuncSetAttribute(mixed_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, MixSmem<128>::kTotal);
-    return cudaFuncSetAttribute(mixed_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, MixSmem<64>::kTotal);
+        return cudaFuncSetAttribute(mixed_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, MixSmem<128>::kTotal);
+    return cudaFuncSetAttribute(mixed_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, MixSmem<64>::kTotal);
 }
 
 }  // namespace ss

@@ -3,7 +3,10 @@
 // The warp kernel is the library's in-CUDA fallback for shapes the tensor-core kernels do not cover and
 // a debugging second opinion (ss_debug_force_simple_path); it is NOT the fast path and never a CPU
 // fallback.  Same definition as everywhere: row j of request r sees keys 0..u_r+j.
+#include <cuda_fp16.h>
+
 #include "common.cuh"
+#include "ptx.cuh"
 
 namespace ss {
 
@@ -12,10 +15,19 @@ constexpr float kLn2 = 0.6931471805599453f;
 
 __device__ __forceinline__ float bf16_bits_to_float(uint32_t hi16) { return __uint_as_float(hi16 << 16); }
 
-template <int D>
+// two E4M3 codes (low 16 bits) -> two floats, exact
+__device__ __forceinline__ float2 e4m3x2_to_float2(uint32_t pair) {
+    const uint32_t h2 = ptx::e4m3x2_to_f16x2(pair);
+    return __half22float2(*reinterpret_cast<const __half2*>(&h2));
+}
+
+// FP8: the caches hold E4M3 codes (one byte per element) with one fp32 scale per (tensor, kv head): K = code * k_scale[g]
+// (folded into the score scale), V = code * v_scale[g] (folded into the final normalisation).  DESIGN.md reading 23.
+template <int D, bool FP8>
 __global__ void __launch_bounds__(128)
-simple_attention_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k_cache,
-                        const __nv_bfloat16* __restrict__ v_cache, const int32_t* __restrict__ block_table,
+simple_attention_kernel(const __nv_bfloat16* __restrict__ q, const void* __restrict__ k_cache_v,
+                        const void* __restrict__ v_cache_v, const float* __restrict__ k_scale,
+                        const float* __restrict__ v_scale, const int32_t* __restrict__ block_table,
                         const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int T,
                         int Hq, int Hkv, int max_pages, float scale, __nv_bfloat16* __restrict__ out,
                         float* __restrict__ lse, int prefill_only) {
@@ -41,7 +53,11 @@ simple_attention_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
     for (int d = lane; d < D; d += 32) s_q[warp][d] = __bfloat162float(qrow[d]);
     __syncwarp();
 
-    const float sl2 = scale * kLog2e;
+    const __nv_bfloat16* k_cache = static_cast<const __nv_bfloat16*>(k_cache_v);
+    const __nv_bfloat16* v_cache = static_cast<const __nv_bfloat16*>(v_cache_v);
+    const uint8_t* k_codes = static_cast<const uint8_t*>(k_cache_v);
+    const uint8_t* v_codes = static_cast<const uint8_t*>(v_cache_v);
+    const float sl2 = scale * kLog2e * (FP8 ? __ldg(k_scale + g) : 1.f);
     float m = -INFINITY, l = 0.f, acc[EPL];
 #pragma unroll
     for (int e = 0; e < EPL; ++e) acc[e] = 0.f;
@@ -54,8 +70,20 @@ simple_attention_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
         if (valid) {
             const int64_t page = __ldg(bt + (t >> 4));
             row_off = ((page * Hkv + g) * kPage + (t & 15)) * (int64_t)D;
-            const uint4* kr = reinterpret_cast<const uint4*>(k_cache + row_off);
             float dot = 0.f;
+            if (FP8) {
+                const uint2* kr = reinterpret_cast<const uint2*>(k_codes + row_off);
+#pragma unroll 4
+                for (int v = 0; v < D / 8; ++v) {
+                    const uint2 w = __ldg(kr + v);
+                    const float* qq = &s_q[warp][v * 8];
+                    const float2 a = e4m3x2_to_float2(w.x), b = e4m3x2_to_float2(w.x >> 16);
+                    const float2 c = e4m3x2_to_float2(w.y), d = e4m3x2_to_float2(w.y >> 16);
+                    dot += qq[0] * a.x + qq[1] * a.y + qq[2] * b.x + qq[3] * b.y;
+                    dot += qq[4] * c.x + qq[5] * c.y + qq[6] * d.x + qq[7] * d.y;
+                }
+            } else {
+            const uint4* kr = reinterpret_cast<const uint4*>(k_cache + row_off);
 #pragma unroll 4
             for (int v = 0; v < D / 8; ++v) {
                 const uint4 w = __ldg(kr + v);
@@ -64,6 +92,7 @@ simple_attention_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
                 dot += qq[2] * bf16_bits_to_float(w.y & 0xffffu) + qq[3] * bf16_bits_to_float(w.y >> 16);
                 dot += qq[4] * bf16_bits_to_float(w.z & 0xffffu) + qq[5] * bf16_bits_to_float(w.z >> 16);
                 dot += qq[6] * bf16_bits_to_float(w.w & 0xffffu) + qq[7] * bf16_bits_to_float(w.w >> 16);
+            }
             }
             s = dot * sl2;
         }
@@ -84,12 +113,19 @@ simple_attention_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16
         for (int i = 0; i < cnt; ++i) {
             const float pi = __shfl_sync(0xffffffffu, p, i);
             const int64_t off = __shfl_sync(0xffffffffu, row_off, i);
-            const __nv_bfloat16* vr = v_cache + off + lane * EPL;
+            if (FP8) {
+                static_assert(!FP8 || EPL == 4, "FP8 path: 4 codes per lane");
+                const float2 a = e4m3x2_to_float2(*reinterpret_cast<const uint32_t*>(v_codes + off + lane * EPL));
+                const float2 b = e4m3x2_to_float2(*reinterpret_cast<const uint32_t*>(v_codes + off + lane * EPL) >> 16);
+                acc[0] += pi * a.x; acc[1] += pi * a.y; acc[2 % EPL] += pi * b.x; acc[3 % EPL] += pi * b.y;
+            } else {
+                const __nv_bfloat16* vr = v_cache + off + lane * EPL;
 #pragma unroll
-            for (int e = 0; e < EPL; ++e) acc[e] += pi * __bfloat162float(vr[e]);
+                for (int e = 0; e < EPL; ++e) acc[e] += pi * __bfloat162float(vr[e]);
+            }
         }
     }
-    const float inv = 1.f / l;
+    const float inv = (FP8 ? __ldg(v_scale + g) : 1.f) / l;
     __nv_bfloat16* orow = out + ((int64_t)row * Hq + h) * D + lane * EPL;
 #pragma unroll
     for (int e = 0; e < EPL; ++e) orow[e] = __float2bfloat16_rn(acc[e] * inv);
@@ -102,14 +138,18 @@ cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_
     const ss_config& c = h->cfg;
     const int64_t units = (int64_t)T * c.num_q_heads;
     const unsigned blocks = (unsigned)((units + 3) / 4);
-    if (c.head_dim == 128)
-        simple_attention_kernel<128><<<blocks, 128, 0, stream>>>(
-            (const __nv_bfloat16*)q, (const __nv_bfloat16*)h->k_cache, (const __nv_bfloat16*)h->v_cache, bt, qsl,
-            ctx, R, T, c.num_q_heads, c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
+    if (h->kv_fp8)
+        simple_attention_kernel<128, true><<<blocks, 128, 0, stream>>>(
+            (const __nv_bfloat16*)q, h->k_cache, h->v_cache, h->k_scale, h->v_scale, bt, qsl, ctx, R, T, c.num_q_heads,
+            c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
+    else if (c.head_dim == 128)
+        simple_attention_kernel<128, false><<<blocks, 128, 0, stream>>>(
+            (const __nv_bfloat16*)q, h->k_cache, h->v_cache, nullptr, nullptr, bt, qsl, ctx, R, T, c.num_q_heads,
+            c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
     else
-        simple_attention_kernel<64><<<blocks, 128, 0, stream>>>(
-            (const __nv_bfloat16*)q, (const __nv_bfloat16*)h->k_cache, (const __nv_bfloat16*)h->v_cache, bt, qsl,
-            ctx, R, T, c.num_q_heads, c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
+        simple_attention_kernel<64, false><<<blocks, 128, 0, stream>>>(
+            (const __nv_bfloat16*)q, h->k_cache, h->v_cache, nullptr, nullptr, bt, qsl, ctx, R, T, c.num_q_heads,
+            c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
     return cudaGetLastError();
 }
 

@@ -70,6 +70,9 @@ struct Handle {
     int32_t* state;                  // device: [0..3] self-cleaning queue tickets, [4..7] debug-check record (code, request,
                                      // value, limit), [8..) split arrival counters (max_requests*Hkv)
     size_t state_bytes;
+    int kv_fp8;                      // SS_FLAG_KV_FP8: caches hold E4M3 codes, one byte per element
+    const float* k_scale;            // device, [Hkv] (ss_set_kv_scales); null until set
+    const float* v_scale;
     int debug_checks;                // SS_FLAG_DEBUG_CHECKS: validate device metadata before every hot call
     unsigned long long* trace;       // ss_debug_set_trace buffer (device) or null
     int trace_words;
@@ -130,7 +133,7 @@ cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_
                                     const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
                                     cudaStream_t stream, int prefill_only = 0);
 bool main_self_plans(const Handle* h, int R, int T);
-cudaError_t init_main_attention(int head_dim);           // one-time function attributes (ss_create)
+cudaError_t init_main_attention(int head_dim, int kv_fp8);   // one-time function attributes (ss_create)
 // SS_FLAG_DEBUG_CHECKS: device-side validation of (qsl, ctx_lens, block_table); records the first violation in
 // h->state[kStateErr..] - the hot kernels of this and later calls then skip every cache / output access
 cudaError_t launch_validate(const Handle* h, const int32_t* bt, const int32_t* qsl, const int32_t* ctx, int R, int T,

@@ -54,7 +54,7 @@ __device__ __forceinline__ int plan_decode_chunk(int n, int L) {
 template <int NT, typename OffT>
 __device__ void build_plan(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int Hq, int Hkv,
                            int D, int num_sms, int force_split_keys, int force_decode_ctas, int32_t* scratch,
-                           PlanTables<OffT> tb, PlanHeader* ph) {
+                           PlanTables<OffT> tb, PlanHeader* ph, int skip_prefill = 0) {
     int32_t* s_c = scratch;
     int32_t* s_u = scratch + R;
     int32_t* s_cost = scratch + 2 * ((R + 3) & ~3);          // 16-byte aligned: read as int4
@@ -65,7 +65,8 @@ __device__ void build_plan(const int32_t* __restrict__ qsl, const int32_t* __res
     unsigned long long my_keys = 0, my_pairs = 0;
     int my_p = 0, my_d = 0;
     for (int r = tid; r < R; r += NT) {
-        const int c = __ldg(qsl + r + 1) - __ldg(qsl + r);
+        int c = __ldg(qsl + r + 1) - __ldg(qsl + r);
+        if (skip_prefill && c > 1) c = 0;                 // FP8 cache: prefill chunks are served by another kernel
         const int u = __ldg(ctx_lens + r);
         s_c[r] = c;
         s_u[r] = u;

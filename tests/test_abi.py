@@ -67,7 +67,10 @@ def test_null_arguments_are_rejected_without_a_device(lib):
     assert lib.ss_kv_append(None, None, None, None, None, None, 1, 1, None) == -1
     assert lib.ss_workspace_bytes(None) == 0
     assert lib.ss_poll_device_error(None, None) == -1 and lib.ss_reset(None, None) == -1
-    bad = ss_config(32, 8, 128, 16, 64, 4, 64, 8, 2)         # unknown flag bit
+    assert lib.ss_set_kv_scales(None, None, None) == -1
+    bad = ss_config(32, 8, 128, 16, 64, 4, 64, 8, 4)         # unknown flag bit
+    assert lib.ss_create(ctypes.byref(h), ctypes.byref(bad), 256, 512) == -1
+    bad = ss_config(8, 8, 64, 16, 64, 4, 64, 8, 2)           # SS_FLAG_KV_FP8 needs head_dim 128
     assert lib.ss_create(ctypes.byref(h), ctypes.byref(bad), 256, 512) == -1
     bad = ss_config(64, 8, 128, 16, 64, 2048, 2 ** 31 - 1, 2 ** 26)   # worst-case item count overflows int32
     assert lib.ss_create(ctypes.byref(h), ctypes.byref(bad), 256, 512) == -1

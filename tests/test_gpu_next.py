@@ -113,3 +113,109 @@ def test_rope_theta_must_be_finite_and_above_one():
         with pytest.raises(binding.SlidingAttnError) as ei:
             h.qkv_rope_append(qkv, dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens), bad)
         assert ei.value.status == binding.SS_ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# NEXT-3: FP8 E4M3 KV cache (a1 quantising append, a4 decode over FP8 tiles, prefill rows by the plain kernel)
+# ------------------------------------------------------------------------------------------------------------------
+def fp8_scales(Hkv, seed):
+    rng = np.random.default_rng(seed)
+    return (rng.uniform(0.008, 0.02, size=Hkv).astype(np.float32), rng.uniform(0.008, 0.02, size=Hkv).astype(np.float32))
+
+
+def quantise_pool(cache_bf16, scale):
+    """Initial cache contents (an INPUT of the test, any codes would do): the N(0,1) pool quantised with torch, poisoned
+    unused slots (bf16 NaN) become E4M3 NaN codes."""
+    s = torch.from_numpy(scale).to(cache_bf16.device).view(1, -1, 1, 1)
+    return (cache_bf16.float() / s).clamp(-448.0, 448.0).to(torch.float8_e4m3fn).view(torch.uint8).contiguous()
+
+
+def fp8_case(b, seed=0, check_rows=None):
+    t = wl.make_tensors(b, DEV, poison_unused=True)
+    ks, vs = fp8_scales(b.num_kv_heads, 500 + seed)
+    kc, vc = quantise_pool(t.k_cache, ks), quantise_pool(t.v_cache, vs)
+    k0, v0 = kc.cpu().numpy().copy(), vc.cpu().numpy().copy()
+    h = binding.handle_for(b, t, fp8_caches=(kc, vc), kv_scales=(dev(ks), dev(vs)))
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    if b.with_append:
+        binding.kv_append(h, t.k_new, t.v_new, bt, qsl, ctx)
+        oracle.kv_append_fp8(k0, v0, wl.to_u16(t.k_new), wl.to_u16(t.v_new), ks, vs, b.block_table, b.query_start_loc, b.ctx_lens)
+    out = binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale)
+    torch.cuda.synchronize()
+    if b.with_append:
+        assert np.array_equal(kc.cpu().numpy(), k0), "FP8 k_cache codes differ from the oracle's"
+        assert np.array_equal(vc.cpu().numpy(), v0), "FP8 v_cache codes differ from the oracle's"
+    rows = None if check_rows is None else np.asarray(check_rows, dtype=np.int32)
+    ref, _ = oracle.mixed_attention_fp8(wl.to_u16(t.q), k0, v0, ks, vs, b.block_table, b.query_start_loc, b.ctx_lens, b.scale, rows=rows)
+    if rows is None:
+        check_attention(b, out, ref)
+    else:
+        got = out.to(torch.float64).cpu().numpy()
+        assert not np.isnan(got).any()
+        err = np.abs(got[rows] - ref)
+        assert err.max() <= MAX_ABS and err.mean() <= MEAN_ABS, (err.max(), err.mean())
+        rel = np.linalg.norm(got[rows] - ref, axis=(1, 2)) / np.maximum(np.linalg.norm(ref, axis=(1, 2)), 1e-30)
+        assert rel.max() <= REL_L2, rel.max()
+    return h
+
+
+def test_fp8_append_every_bf16_pattern():
+    """Quantisation decision on every bf16 input (NaN payloads, +-inf, denormals, -0, ties) at several scales: bit-exact."""
+    Hkv, D = 2, 128
+    pats = np.arange(65536, dtype=np.uint16)
+    T = 65536 // (Hkv * D)
+    b = wl.make_batch("fp8-all", 4, Hkv, D, [(T, 5)], 77, with_append=True)
+    t = wl.make_tensors(b, DEV)
+    k_new = torch.from_numpy(pats.view(np.int16).reshape(T, Hkv, D).copy()).to(DEV).view(torch.bfloat16)
+    v_new = torch.from_numpy(np.roll(pats, 12345).view(np.int16).reshape(T, Hkv, D).copy()).to(DEV).view(torch.bfloat16)
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    for scales in ([1.0, 0.0123], [3.7, 2.0 ** -10], [1e-3, 448.0], [0.3333333, 1e-30]):
+        ks, vs = np.asarray(scales, dtype=np.float32), np.asarray(scales[::-1], dtype=np.float32)
+        kc = torch.full(t.k_cache.shape, 0x55, dtype=torch.uint8, device=DEV)
+        vc = torch.full(t.v_cache.shape, 0xAA, dtype=torch.uint8, device=DEV)
+        k0, v0 = kc.cpu().numpy().copy(), vc.cpu().numpy().copy()
+        h = binding.handle_for(b, t, fp8_caches=(kc, vc), kv_scales=(dev(ks), dev(vs)))
+        binding.kv_append(h, k_new, v_new, bt, qsl, ctx)
+        torch.cuda.synchronize()
+        oracle.kv_append_fp8(k0, v0, wl.to_u16(k_new), wl.to_u16(v_new), ks, vs, b.block_table, b.query_start_loc, b.ctx_lens)
+        assert np.array_equal(kc.cpu().numpy(), k0) and np.array_equal(vc.cpu().numpy(), v0), f"scales {scales}"
+
+
+@pytest.mark.parametrize("shape", [(8, 2, 128), (28, 4, 128), (32, 8, 128), (64, 8, 128), (16, 1, 128), (4, 4, 128)])
+def test_fp8_random_mixed_batches(shape):
+    Hq, Hkv, D = shape
+    for seed in (0, 1):
+        b = wl.random_batch(4100 + 11 * seed + Hq, Hq=Hq, Hkv=Hkv, D=D, n_prefill=2, n_decode=9, max_c=150, max_u=1500)
+        fp8_case(wl.Batch(**{**b.__dict__, "with_append": True}), seed)
+
+
+def test_fp8_decode_long_contexts_and_splits():
+    """Split-KV over FP8 tiles: contexts to 12 345 keys (several splits), ragged tails, a single cached key."""
+    reqs = [(1, 12345), (1, 4095), (1, 4096), (1, 63), (1, 64), (1, 65), (1, 0), (1, 1), (1, 15), (1, 16), (1, 8191), (1, 777)]
+    fp8_case(wl.make_batch("fp8-long", 32, 8, 128, reqs, 78, with_append=True))
+    fp8_case(wl.make_batch("fp8-long-g8", 64, 8, 128, reqs, 79, with_append=True), 1)
+
+
+def test_fp8_pure_decode_batch_all_rows():
+    b = wl.config_c3(0, 1, 128)                          # PD-128: 128 decodes, lognormal contexts
+    fp8_case(wl.Batch(**{**b.__dict__, "with_append": True}))
+
+
+def test_fp8_needs_scales_and_head_dim_128():
+    b = wl.make_batch("fp8-bad", 8, 2, 128, [(1, 5)], 80, with_append=True)
+    t = wl.make_tensors(b, DEV)
+    kc = torch.zeros(t.k_cache.shape, dtype=torch.uint8, device=DEV)
+    h = binding.handle_for(b, t, fp8_caches=(kc, kc.clone()))
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    with pytest.raises(binding.SlidingAttnError) as ei:
+        binding.kv_append(h, t.k_new, t.v_new, bt, qsl, ctx)
+    assert ei.value.status == binding.SS_ERR_INVALID_ARG
+    with pytest.raises(binding.SlidingAttnError) as ei:
+        binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale)
+    assert ei.value.status == binding.SS_ERR_INVALID_ARG
+    b64 = wl.config_tiny()
+    t64 = wl.make_tensors(b64, DEV)
+    kc64 = torch.zeros(t64.k_cache.shape, dtype=torch.uint8, device=DEV)
+    with pytest.raises(binding.SlidingAttnError) as ei:
+        binding.handle_for(b64, t64, fp8_caches=(kc64, kc64.clone()))
+    assert ei.value.status == binding.SS_ERR_INVALID_ARG
