@@ -7,8 +7,9 @@ A "step" = one pass of the whole hot path over one synthetic batch: kv_append of
 Headline workload at N=1: BASELINE.json configs[4] "C5" — the largest MIXED single-GPU configuration
 (Llama-3-70B-shaped layer, 2 x 1024 chunk tokens + 192 decodes, with append), which runs every row of
 SURVEY.md §8(a).  The same line carries `per_config`: C2 (configs[1]), C4 (configs[3], decode-heavy, the
->= 70 % HBM target), PP-b / PP-f (chunk-heavy scene edges, the >= 50 % tensor target) and PD-32 (small
-pure-decode call), each timed with the same protocol and with its own roofline object.  Other workloads:
+>= 70 % HBM target), C4/fp8 (the same batch over an FP8 E4M3 KV cache: half the algorithmic KV bytes), PP-b / PP-f
+(chunk-heavy scene edges, the >= 50 % tensor target) and PD-32 (small pure-decode call), each timed with the same
+protocol and with its own roofline object.  Other workloads:
 --workload NAME; --per-config a,b,c or "none".
 
 Metric: BASELINE.json's "mixed prefill+decode attention us/iter and % of HBM/tensor roofline" -> value =
@@ -40,11 +41,14 @@ sys.path.insert(0, str(ROOT))
 METRIC = "mixed prefill+decode attention us/iter and % of HBM/tensor roofline"
 UNIT = "us/iter"
 HEADLINE = "C5"
-PER_CONFIG = "C2,C4,PP-b,PP-f,PD-32"
+PER_CONFIG = "C2,C4,C4/fp8,PP-b,PP-f,PD-32"
 
 
 def get_batch(name: str):
     from paper_2606_05933_b200 import workloads as wl
+    if name.endswith("/fp8"):                       # the same batch over an FP8 E4M3 KV cache (SS_FLAG_KV_FP8)
+        b = get_batch(name[:-4])
+        return wl.Batch(**{**b.__dict__, "name": b.name + "/fp8", "meta": {**b.meta, "kv_fp8": True}})
     if name == "C1":
         return wl.config_tiny()
     if name == "C2":
@@ -274,8 +278,13 @@ class Bench:
         from paper_2606_05933_b200 import binding, workloads as wl
         self.name, self.devname = name, devname
         self.b = get_batch(name)
-        self.t = wl.make_tensors(self.b, devname)
-        self.h = binding.handle_for(self.b, self.t)
+        if self.b.meta.get("kv_fp8"):
+            self.t = wl.make_tensors(self.b, devname, caches=False)
+            kc, vc, ks, vs = wl.make_fp8_caches(self.b, devname)
+            self.h = binding.handle_for(self.b, self.t, fp8_caches=(kc, vc), kv_scales=(ks, vs))
+        else:
+            self.t = wl.make_tensors(self.b, devname)
+            self.h = binding.handle_for(self.b, self.t)
         to_dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(devname)
         self.bt, self.qsl, self.ctx = to_dev(self.b.block_table), to_dev(self.b.query_start_loc), to_dev(self.b.ctx_lens)
         self.out = torch.empty_like(self.t.q)

@@ -1,6 +1,7 @@
 """Algorithmic work of one mixed_attention iteration.
 
-bytes = every visible K and V row once + Q in + O out;  flops = 4*D*Hq*pairs.  Block tables, the
+bytes = every visible K and V row once (2 bytes per element, 1 for an FP8 cache: batch.meta["kv_fp8"]) + Q in +
+O out;  flops = 4*D*Hq*pairs.  Block tables, the
 work list and split partials are excluded (they are the implementation's, not the method's)."""
 from __future__ import annotations
 
@@ -30,17 +31,18 @@ def work(batch) -> Dict[str, float]:
     reqs = [(c, u) for c, u in batch.reqs if c > 0]
     kv_tokens = sum(c + u for c, u in reqs)
     T = sum(c for c, _ in reqs)
-    kv_bytes = kv_tokens * 2 * Hkv * D * 2
+    esz = 1 if batch.meta.get("kv_fp8") else 2       # bytes per cached element (FP8 E4M3 cache: 1)
+    kv_bytes = kv_tokens * 2 * Hkv * D * esz
     qo_bytes = 2 * T * Hq * D * 2
     pairs = causal_pairs(reqs)
     Dset, Pset = split_sets(reqs)
     pairs_P = causal_pairs([reqs[i] for i in Pset])
-    kv_bytes_D = sum(reqs[i][0] + reqs[i][1] for i in Dset) * 2 * Hkv * D * 2
+    kv_bytes_D = sum(reqs[i][0] + reqs[i][1] for i in Dset) * 2 * Hkv * D * esz
     return {
         "kv_bytes": kv_bytes, "qo_bytes": qo_bytes, "bytes": kv_bytes + qo_bytes,
         "flops": 4 * D * Hq * pairs, "pairs": pairs,
         "prefill_flops": 4 * D * Hq * pairs_P, "decode_kv_bytes": kv_bytes_D,
-        "append_bytes": 4 * T * Hkv * D * 2 if batch.with_append else 0,
+        "append_bytes": 2 * T * Hkv * D * (2 + esz) if batch.with_append else 0,
     }
 
 

@@ -304,30 +304,32 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
 #pragma unroll
                 for (int i = 0; i < 4; ++i) sT[nt][i] = sU[nt][i] = 0.f;
             const int rk = r16 + (mi & 1) * 8 + l7;          // a0: keys 0-7, a1: keys 8-15, a2 / a3: the next 8 d
+            // every fragment load is issued before the first MMA (the wrappers are asm volatile and keep their order: an
+            // interleaved loop exposed one ldmatrix latency per k-step)
             if (FP8) {
+                uint32_t r[D / 32][4];                           // one ldmatrix = 16 keys x 32 d of codes = two k-steps
 #pragma unroll
-                for (int jj = 0; jj < D / 32; ++jj) {            // one ldmatrix = 16 keys x 32 d of codes = two k-steps
-                    const int cd = 2 * jj + (mi >> 1);
-                    uint32_t r[4];
-                    ldmatrix_x4(r[0], r[1], r[2], r[3], kbase + SM::kv_off(rk, cd));
+                for (int jj = 0; jj < D / 32; ++jj)
+                    ldmatrix_x4(r[jj][0], r[jj][1], r[jj][2], r[jj][3], kbase + SM::kv_off(rk, 2 * jj + (mi >> 1)));
+#pragma unroll
+                for (int jj = 0; jj < D / 32; ++jj)
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         const int ks = 2 * jj + h;
-                        const uint32_t a[4] = {e4m3x2_to_f16x2(r[2 * h]), e4m3x2_to_f16x2(r[2 * h + 1]),
-                                               e4m3x2_hi_to_f16x2(r[2 * h]), e4m3x2_hi_to_f16x2(r[2 * h + 1])};
+                        const uint32_t a[4] = {e4m3x2_to_f16x2(r[jj][2 * h]), e4m3x2_to_f16x2(r[jj][2 * h + 1]),
+                                               e4m3x2_hi_to_f16x2(r[jj][2 * h]), e4m3x2_hi_to_f16x2(r[jj][2 * h + 1])};
 #pragma unroll
                         for (int nt = 0; nt < NT; ++nt) mma_f16_16816(h ? sU[nt] : sT[nt], a, qb[ks][2 * nt], qb[ks][2 * nt + 1]);
                     }
-                }
             } else {
+                uint32_t a[D / 16][4];
 #pragma unroll
-            for (int ks = 0; ks < D / 16; ++ks) {
-                const int cd = 2 * ks + (mi >> 1);
-                uint32_t a[4];
-                ldmatrix_x4(a[0], a[1], a[2], a[3], kbase + SM::kv_off(rk, cd));
+                for (int ks = 0; ks < D / 16; ++ks)
+                    ldmatrix_x4(a[ks][0], a[ks][1], a[ks][2], a[ks][3], kbase + SM::kv_off(rk, 2 * ks + (mi >> 1)));
 #pragma unroll
-                for (int nt = 0; nt < NT; ++nt) mma_bf16_16816((ks & 1) ? sU[nt] : sT[nt], a, qb[ks][2 * nt], qb[ks][2 * nt + 1]);
-            }
+                for (int ks = 0; ks < D / 16; ++ks)
+#pragma unroll
+                    for (int nt = 0; nt < NT; ++nt) mma_bf16_16816((ks & 1) ? sU[nt] : sT[nt], a[ks], qb[ks][2 * nt], qb[ks][2 * nt + 1]);
             }
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt)
@@ -349,6 +351,17 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
                     asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(a), "r"(0u) : "memory");
                 }
                 __syncwarp();
+            }
+            // the V fragments are requested now, ahead of the softmax arithmetic that hides their latency.
+            // bf16: a0 = (keys 0-7, d 0-7)^T, a1 = (keys 0-7, d 8-15)^T, a2 / a3: keys 8-15, one ldmatrix per 16 d;
+            // FP8: matrices (keys 0-7, chunk), (keys 8-15, chunk), the same for chunk + 1, one ldmatrix per 32 d
+            constexpr int kVLoads = FP8 ? D / 32 : D / 16;
+            uint32_t va[kVLoads][4];
+            {
+                const int rv = r16 + (FP8 ? (mi & 1) : (mi >> 1)) * 8 + l7;
+#pragma unroll
+                for (int i = 0; i < kVLoads; ++i)
+                    ldmatrix_x4_trans(va[i][0], va[i][1], va[i][2], va[i][3], vbase + SM::kv_off(rv, 2 * i + (FP8 ? (mi >> 1) : (mi & 1))));
             }
             uint32_t pb[NT][2];                              // B fragments of P^T (16 keys x 8 heads)
             bool moved = false;
@@ -389,33 +402,23 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
             }
 #pragma unroll
             for (int nt = 0; nt < NT; ++nt) { l[nt][0] += sT[nt][0]; l[nt][1] += sT[nt][1]; }
-            // O^T (D x 8 heads) += V^T (D x 16 keys) P^T: a0 = (keys 0-7, d 0-7)^T, a1 = (keys 0-7, d 8-15)^T, a2 / a3: keys 8-15
+            // O^T (D x 8 heads) += V^T (D x 16 keys) P^T
             if (FP8) {
-                const int rv = r16 + (mi & 1) * 8 + l7;          // matrices: (keys 0-7, chunk), (keys 8-15, chunk), the same for chunk + 1
 #pragma unroll
-                for (int mm = 0; mm < D / 32; ++mm) {
-                    const int cd = 2 * mm + (mi >> 1);
-                    uint32_t r[4];
-                    ldmatrix_x4_trans(r[0], r[1], r[2], r[3], vbase + SM::kv_off(rv, cd));
+                for (int mm = 0; mm < D / 32; ++mm)
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
                         // register = codes [key 2c][d 2qr], [2c][2qr+1], [2c+1][2qr], [2c+1][2qr+1] -> (d 2qr | d 2qr+1) x keys (2c, 2c+1)
-                        const uint32_t x0 = __byte_perm(r[2 * h], 0u, 0x3120), x1 = __byte_perm(r[2 * h + 1], 0u, 0x3120);
+                        const uint32_t x0 = __byte_perm(va[mm][2 * h], 0u, 0x3120), x1 = __byte_perm(va[mm][2 * h + 1], 0u, 0x3120);
                         const uint32_t a[4] = {e4m3x2_to_f16x2(x0), e4m3x2_hi_to_f16x2(x0), e4m3x2_to_f16x2(x1), e4m3x2_hi_to_f16x2(x1)};
 #pragma unroll
                         for (int nt = 0; nt < NT; ++nt) mma_f16_16816(oT[nt][2 * mm + h], a, pb[nt][0], pb[nt][1]);
                     }
-                }
             } else {
-            const int rv = r16 + (mi >> 1) * 8 + l7;
 #pragma unroll
-            for (int mt = 0; mt < D / 16; ++mt) {
-                const int cd = 2 * mt + (mi & 1);
-                uint32_t a[4];
-                ldmatrix_x4_trans(a[0], a[1], a[2], a[3], vbase + SM::kv_off(rv, cd));
+                for (int mt = 0; mt < D / 16; ++mt)
 #pragma unroll
-                for (int nt = 0; nt < NT; ++nt) mma_bf16_16816(oT[nt][mt], a, pb[nt][0], pb[nt][1]);
-            }
+                    for (int nt = 0; nt < NT; ++nt) mma_bf16_16816(oT[nt][mt], va[mt], pb[nt][0], pb[nt][1]);
             }
             if (nvalid < kDecKeys) fence_proxy_async();
         }

@@ -83,12 +83,19 @@ def surface_points(with_c4: bool = False, dense: bool = False, model: Optional[s
         pts.append((name, lambda name=name: wl.config_scene_edge(name)))
     for name in ("PD-32", "PD-128", "PD-C2", "PD-C5"):     # pure-decode scene edges
         pts.append((name, lambda name=name: wl.config_decode_only(name)))
+    for name in ("PD-32", "PD-128", "PD-C2", "PD-C5"):     # the same pure-decode edges over an FP8 E4M3 KV cache (NEXT-3)
+        pts.append((name + "/fp8", lambda name=name: fp8_variant(wl.config_decode_only(name))))
     pts.append(("C2", wl.config_c2))
     pts.append(("C2-shuffled", lambda: wl.config_c2(shuffle=True)))
     pts.append(("C5", wl.config_c5))
     if with_c4:
         pts.append(("C4", wl.config_c4))
+        pts.append(("C4/fp8", lambda: fp8_variant(wl.config_c4())))
     return pts
+
+
+def fp8_variant(b: wl.Batch) -> wl.Batch:
+    return wl.Batch(**{**b.__dict__, "name": b.name + "/fp8", "meta": {**b.meta, "kv_fp8": True}})
 
 
 def sub_batch(b: wl.Batch, kind: str) -> Optional[wl.Batch]:
@@ -104,8 +111,13 @@ def time_batch(b: wl.Batch, device: str, iters: int, warmup: int, flush) -> np.n
     """us per ss_mixed_attention call (work list + main launch), one sample per timed iteration."""
     import torch
     from . import binding
-    t = wl.make_tensors(b, device)
-    h = binding.handle_for(b, t)
+    if b.meta.get("kv_fp8"):
+        t = wl.make_tensors(b, device, caches=False)
+        kc, vc, ks, vs = wl.make_fp8_caches(b, device)
+        h = binding.handle_for(b, t, fp8_caches=(kc, vc), kv_scales=(ks, vs))
+    else:
+        t = wl.make_tensors(b, device)
+        h = binding.handle_for(b, t)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
     bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
     out = torch.empty_like(t.q)

@@ -274,7 +274,32 @@ def _randn_bf16(shape, gen: torch.Generator, device, chunk_elems: int = 1 << 27)
     return out.view(*shape)
 
 
-def make_tensors(b: Batch, device="cpu", poison_unused: bool = False) -> Tensors:
+def make_fp8_caches(b: Batch, device, seed_offset: int = 0):
+    """FP8 E4M3 cache pools for timing runs (SS_FLAG_KV_FP8): uniformly random codes, the two NaN codes (0x7F, 0xFF)
+    mapped to zero, and per kv head fp32 scales in [0.008, 0.02] (code magnitudes are log-uniform over 2^-9 .. 448, so
+    values reach ~ +-9).  Pure input generation: no quantisation arithmetic lives here.
+    Returns (k_codes, v_codes, k_scale, v_scale), caches uint8 [P,Hkv,page,D], scales float32 [Hkv] on `device`."""
+    device = torch.device(device)
+    gen = torch.Generator(device=device)
+    gen.manual_seed(1000003 * b.seed + 29 + seed_offset)
+    shape = (b.num_pages, b.num_kv_heads, b.page_size, b.head_dim)
+    caches = []
+    for _ in range(2):
+        c = torch.empty(shape, dtype=torch.uint8, device=device)
+        flat = c.view(-1)
+        for s in range(0, flat.numel(), 1 << 28):
+            e = min(flat.numel(), s + (1 << 28))
+            r = torch.randint(0, 256, (e - s,), generator=gen, device=device, dtype=torch.int16)
+            r[(r & 0x7F) == 0x7F] = 0
+            flat[s:e] = r.to(torch.uint8)
+        caches.append(c)
+    rng = np.random.default_rng(b.seed + 4242 + seed_offset)
+    ks = torch.from_numpy(rng.uniform(0.008, 0.02, size=b.num_kv_heads).astype(np.float32)).to(device)
+    vs = torch.from_numpy(rng.uniform(0.008, 0.02, size=b.num_kv_heads).astype(np.float32)).to(device)
+    return caches[0], caches[1], ks, vs
+
+
+def make_tensors(b: Batch, device="cpu", poison_unused: bool = False, caches: bool = True) -> Tensors:
     """N(0,1) bf16 everywhere (every cache page, used or not).  With ``poison_unused`` the slots no
     request may read (pages outside every block table, slots past u+c in last pages) get bf16 NaN /
     +-3e38 bit patterns to prove the path never touches them (SURVEY.md §8(c) reading 7).
@@ -289,6 +314,8 @@ def make_tensors(b: Batch, device="cpu", poison_unused: bool = False) -> Tensors
     k_new = _randn_bf16((T, b.num_kv_heads, b.head_dim), gen, device)
     v_new = _randn_bf16((T, b.num_kv_heads, b.head_dim), gen, device)
     cshape = (b.num_pages, b.num_kv_heads, b.page_size, b.head_dim)
+    if not caches:                                   # FP8 runs bring their own pools (make_fp8_caches)
+        return Tensors(q, k_new, v_new, None, None)
     k_cache = _randn_bf16(cshape, gen, device)
     v_cache = _randn_bf16(cshape, gen, device)
     if poison_unused:
