@@ -326,6 +326,35 @@ class Bench:
         wall = time.perf_counter() - wall0
         return np.array([e0.elapsed_time(e1) for e0, e1 in evs], dtype=np.float64), launches, wall
 
+    def time_graph(self, steps: int, flush) -> float:
+        """Median us per step when the step (append + attention) is replayed from a CUDA graph: same protocol."""
+        import torch
+        from paper_2606_05933_b200 import binding
+        b, t, h = self.b, self.t, self.h
+        g, s = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            binding.kv_append(h, t.k_new, t.v_new, self.bt, self.qsl, self.ctx, stream=s)
+            binding.mixed_attention(h, t.q, self.bt, self.qsl, self.ctx, b.scale, out=self.out, stream=s)
+            s.synchronize()
+            with torch.cuda.graph(g, stream=s):
+                binding.kv_append(h, t.k_new, t.v_new, self.bt, self.qsl, self.ctx, stream=s)
+                binding.mixed_attention(h, t.q, self.bt, self.qsl, self.ctx, b.scale, out=self.out, stream=s)
+        torch.cuda.current_stream().wait_stream(s)
+        stream = torch.cuda.current_stream()
+        us = []
+        for i in range(steps + 3):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            g.replay()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if i >= 3:
+                us.append(e0.elapsed_time(e1) * 1e3)
+        del g
+        return float(np.median(us))
+
     def roofline(self, steps: int, flush, step_ms: float) -> dict:
         """Dominant kernel (the main attention launch, a3+a4+a5) timed by CUDA events inside the library on the same
         stream; algorithmic bytes / flops of the batch over that time vs the measured peak."""
@@ -474,6 +503,8 @@ def run_cuda(args):
                    "steps": pc_steps, "us_per_iter": float(ms.mean() * 1e3), "median_us": float(np.median(ms) * 1e3),
                    "p10_us": float(np.percentile(ms, 10) * 1e3), "p90_us": float(np.percentile(ms, 90) * 1e3),
                    "launches_per_step": int(nl), "roofline": pb.roofline(pc_steps, flush, float(ms.mean()))}
+            if name in ("PD-32", "C2"):
+                ent["graph_replay_median_us"] = pb.time_graph(min(pc_steps, 20), flush)   # the same step replayed from a CUDA graph
             per_config.append(ent)
             pb.close()
 

@@ -118,6 +118,9 @@ def load_surface(path):
     """One CSV path, or several (grid + dense points) to be concatenated."""
     paths = [path] if isinstance(path, str) else list(path)
     rows = [r for p in paths for r in csv.DictReader(open(p))]
+    # one model set per layer shape AND cache type: points measured over an FP8 KV cache (point id .../fp8) move half
+    # the bytes and are left out of the bf16 fit
+    rows = [r for r in rows if r.get("kv_dtype", "fp8" if r["point"].endswith("/fp8") else "bf16") == "bf16"]
     X = np.array([[float(r[f]) for f in FEATURES] for r in rows])
     y = np.array([float(r["median_us"]) for r in rows])
     scenes = [r["scene"] for r in rows]

@@ -25,7 +25,7 @@ from . import accounting as acc
 from . import workloads as wl
 from .features import features, scene
 
-FIELDS = ["point", "name", "seed", "shape", "scene", "R", "T", "chunk", "n_prefill", "n_decode", "ctx_median",
+FIELDS = ["point", "name", "seed", "shape", "kv_dtype", "scene", "R", "T", "chunk", "n_prefill", "n_decode", "ctx_median",
           "x1", "x2", "x3", "x4", "x5", "x6", "x7", "bytes", "flops", "t_hbm_us", "t_tc_us", "roofline_us", "bound",
           "median_us", "p10_us", "p90_us", "frac_of_roofline", "prefill_only_us", "decode_only_us", "overlap"]
 
@@ -166,7 +166,7 @@ def main(argv=None):
             b = make()
             us = time_batch(b, device, args.iters, args.warmup, flush)
             w, roof, x = acc.work(b), acc.roofline_us(b, peaks), features(b.reqs)
-            row = {"point": pid, "name": b.name, "seed": b.seed, "shape": f"{b.num_q_heads}/{b.num_kv_heads}/{b.head_dim}",
+            row = {"point": pid, "name": b.name, "seed": b.seed, "shape": f"{b.num_q_heads}/{b.num_kv_heads}/{b.head_dim}", "kv_dtype": "fp8" if b.meta.get("kv_fp8") else "bf16",
                    "scene": scene(b.reqs), "R": b.R, "T": b.T, "chunk": b.meta.get("chunk", x["x6"]),
                    "n_prefill": sum(1 for c, _ in b.reqs if c > 1), "n_decode": x["x4"],
                    "ctx_median": b.meta.get("ctx_median", ""), **x, "bytes": w["bytes"], "flops": w["flops"],

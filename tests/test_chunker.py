@@ -58,21 +58,64 @@ def test_ternary_search_matches_brute_force_on_the_two_window_objective():
         assert t_star - best <= 0.02 * best + 0.5
 
 
-def test_chunker_on_the_measured_surface():
-    """End to end with the predictor fitted on the committed B200 latency surface.  The unconstrained least-squares fit
-    on this small grid is not monotone in the budget (negative weights on x6 / x7), so only what Algorithm 1 guarantees
-    is asserted: a budget in [|D|, B], an allocation that spends it in sorted order, T* = the two-window objective at
-    B*, and B* no worse than the two ends of the range."""
-    rows, X, y, scenes, shapes = load_surface("profiles/r1_v4_surface.csv")
+def _fitted_forwarder(max_budget):
+    from pathlib import Path
+    prof = Path(__file__).resolve().parent.parent / "profiles"
+    rows, X, y, scenes, shapes = load_surface([str(prof / "r2_surface.csv"), str(prof / "r2_surface_dense.csv")])
     keep = [i for i, s in enumerate(shapes) if s == "32/8/128"]
-    p = BatchLatencyPredictor().fit(X[keep], y[keep], [scenes[i] for i in keep])
-    F = BatchForwarder(surface_predict_fn(p), max_budget=2048)
+    p = BatchLatencyPredictor(fit="nnls").fit(X[keep], y[keep], [scenes[i] for i in keep])
+    return BatchForwarder(surface_predict_fn(p), max_budget=max_budget), p
+
+
+def test_fitted_predictor_is_monotone_in_the_budget_inside_a_scene():
+    """The non-negative fit (reading 16): Pred(b) never decreases as the budget grows while the batch stays
+    in one scene (the expert models of two scenes may disagree at the scene switch b = |D| -> |D| + 1, as the paper's do)."""
+    F, p = _fitted_forwarder(4096)
+    for w in p.experts.values():
+        a = w.weights
+        assert a[0] >= 0 and a[1] >= -0.5 * a[0] - 1e-18 and (a[2:] >= 0).all()
+    rng = np.random.default_rng(5)
+    for trial in range(5):
+        dec = list(rng.integers(200, 6000, size=int(rng.integers(8, 128))))
+        pre = [PrefillState(int(rng.integers(500, 6000)), int(rng.integers(0, 3000))) for _ in range(int(rng.integers(1, 4)))]
+        # a request that is handed exactly 1 token counts as a decode (D = {c_i <= 1}, PAPER.md:111): those budgets
+        # switch features / scene and are left out
+        bs = [b for b in range(len(dec) + 2, 4097, 37) if 1 not in F.forward(dec, pre, b)[1]]
+        t = [F.pred(b, dec, pre) for b in bs]
+        assert all(y2 >= y1 - 1e-9 for y1, y2 in zip(t, t[1:]))
+
+
+def test_chunker_on_the_measured_surface():
+    """End to end with the predictor fitted (non-negative weights) on the committed B200 latency surface: TimeToBudget is
+    the largest feasible budget (brute force over the mixed-scene range), Algorithm 1's result is the two-window
+    objective at B*, never worse than both ends of the range and within the final bracket's resolution of the
+    exhaustive optimum."""
+    F, _ = _fitted_forwarder(4096)
     dec = list(np.random.default_rng(2).integers(200, 6000, size=64))
-    pre = [PrefillState(1800, 0), PrefillState(900, 1024)]
-    for slack in (140.0, 180.0, 250.0, 400.0):
-        b_star, a_star, t_star, b_sigma = sliding_chunker(F, dec, pre, slack, slack + 100.0)
+    pre = [PrefillState(3800, 0), PrefillState(1900, 1024)]
+    lo = len(dec) + 2                                         # first budget of the mixed scene (1 token = a decode)
+    for T in (150.0, 180.0, 250.0, 400.0, 1e9):
+        b = F.time_to_budget(dec, pre, T)
+        feas = [x for x in range(lo, F.B + 1) if F.pred(x, dec, pre) <= T]
+        if feas and F.pred(len(dec), dec, pre) <= T:
+            assert b == max(feas)
+    for slack in (160.0, 180.0, 250.0, 400.0):
+        b_star, a_star, t_star, b_sigma = sliding_chunker(F, dec, pre, slack, slack - 30.0)
         assert len(dec) <= b_star <= F.B
-        assert sum(a_star) == min(b_star - len(dec), 2700) and a_star[0] == min(1800, b_star - len(dec))
+        assert sum(a_star) == min(b_star - len(dec), 5700) and a_star[0] == min(3800, b_star - len(dec))
         two = lambda b: F.pred(b, dec, pre) + F.pred(b_sigma - b, dec, pre)
         assert abs(t_star - two(b_star)) < 1e-9
         assert t_star <= min(two(len(dec)), two(F.B)) + 1e-9
+        best = min(two(b) for b in range(len(dec), F.B + 1, 7))
+        assert t_star - best <= 0.02 * best + 0.5
+
+
+def test_fig1_example_runs_on_the_committed_surface():
+    from paper_2606_05933_b200 import fig1_example as ex
+    dec, pre, B, t_cur, t_next = ex.scenario()
+    F = ex.fitted_forwarder(B)
+    single, sliding, b_sigma = ex.plan(F, dec, pre, t_cur, t_next)
+    assert sum(single) == b_sigma == sum(sliding)
+    two = lambda b: F.pred(b, dec, pre) + F.pred(b_sigma - b, dec, pre)
+    assert two(sliding[0]) <= two(single[0]) + 1e-9            # Eq. 16 on the unchanged (D, P)
+    assert F.pred(single[0], dec, pre) <= t_cur and F.pred(single[1], dec, pre) <= t_next

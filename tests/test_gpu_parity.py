@@ -545,3 +545,38 @@ def test_iteration_host_matches_device_path():
     h2.iteration_host(t_host.q, t_host.k_new, t_host.v_new, torch.from_numpy(b.block_table), torch.from_numpy(b.query_start_loc),
                       torch.from_numpy(b.ctx_lens), b.scale, out_host)
     assert torch.equal(out_host, out_dev.cpu()) and torch.equal(kc, t.k_cache)
+
+
+def test_append_plus_attention_is_cuda_graph_capturable():
+    """One iteration (a1 + a2..a5, programmatic dependent launch between them) captured into a CUDA graph and replayed:
+    nothing on the hot path touches the host besides encoding the Q tensor map from its (fixed) pointer.  The replay
+    must reproduce the eager result bit for bit, also after the inputs changed in place."""
+    b = wl.config_c3(256, 2, 32)
+    b = wl.Batch(**{**b.__dict__, "with_append": True})
+    t = wl.make_tensors(b, DEV)
+    h = binding.handle_for(b, t)
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    out_eager = torch.empty_like(t.q)
+    binding.kv_append(h, t.k_new, t.v_new, bt, qsl, ctx)
+    binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale, out=out_eager)
+    torch.cuda.synchronize()
+    out_graph = torch.zeros_like(t.q)
+    g = torch.cuda.CUDAGraph()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        binding.kv_append(h, t.k_new, t.v_new, bt, qsl, ctx, stream=s)       # warm-up on the capture stream
+        binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale, out=out_graph, stream=s)
+        s.synchronize()
+        with torch.cuda.graph(g, stream=s):
+            binding.kv_append(h, t.k_new, t.v_new, bt, qsl, ctx, stream=s)
+            binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale, out=out_graph, stream=s)
+    out_graph.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out_graph, out_eager)
+    t.q.mul_(-1.0)                                                   # new inputs, same pointers: replay follows them
+    binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale, out=out_eager)
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out_graph, out_eager)
