@@ -188,9 +188,10 @@ __device__ __forceinline__ float softmax_half(uint32_t (&sr)[2][32], int nvis, f
 #pragma unroll
     for (int c = 0; c < 2; ++c)
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
+        for (int i = 0; i < 32; i += 2) {
             if (MASKED && c * 32 + i >= nvis) sr[c][i] = 0xff800000u;   // -inf by select, never by arithmetic
-            bm[i & 3] = fmaxf(bm[i & 3], __uint_as_float(sr[c][i]));
+            if (MASKED && c * 32 + i + 1 >= nvis) sr[c][i + 1] = 0xff800000u;
+            bm[(i >> 1) & 3] = fmax3(bm[(i >> 1) & 3], __uint_as_float(sr[c][i]), __uint_as_float(sr[c][i + 1]));   // FMNMX3
         }
     const float cand = fmaxf(fmaxf(bm[0], bm[1]), fmaxf(bm[2], bm[3])) * sl2;
     // lazy rescale: only move the reference max when it grows by more than 2^8

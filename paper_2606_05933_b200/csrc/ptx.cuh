@@ -136,6 +136,12 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
 }
+// three-input maximum (FMNMX3 on sm_100)
+__device__ __forceinline__ float fmax3(float a, float b, float c) {
+    float d;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+    return d;
+}
 // ---- FP8 E4M3 (OCP e4m3fn) <-> fp16 / fp32 ----
 // two codes (low 16 bits of `pair`: byte 0 -> .x / low half) -> two fp16 values, exact (every e4m3 value is an fp16 value)
 __device__ __forceinline__ uint32_t e4m3x2_to_f16x2(uint32_t pair) {
