@@ -56,7 +56,8 @@ using namespace ptx;
 
 constexpr int kMixThreads = 384;
 constexpr int kSlotKeys = 64;        // keys per K / V ring slot = keys per S buffer
-constexpr int kNumSt = 5;            // K ring slots = V ring slots (4: -1.5 % on pure decode, 6 would not leave room for 2 Q tiles)
+constexpr int kMaxSt = 8;            // most K / V ring slots of any instantiation (barrier index layout)
+constexpr int kBarBytes = 640;       // mbarrier block (8 bytes each)
 constexpr int kSchedSlots = 4;
 constexpr int kDecKeys = 16;         // keys of a 64-key slot one decode warp owns (4 warps per slot)
 // setmaxnreg moves registers inside the CTA's own launch allocation: 384 threads x 168 (the __launch_bounds__ cap ptxas
@@ -68,13 +69,19 @@ constexpr float kMLog2e = 1.4426950408889634f;
 constexpr float kMLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.f;   // log2 units: P <= 2^8, safe in bf16 / fp32
 
-// FP8: the KV cache holds one byte per element (E4M3 codes): a key row is D bytes = D/128 128-byte chunks; the ring
-// keeps the bf16 slot size (half of each slot stays unused) so every other offset is the same in both instantiations.
+// FP8: the KV cache holds one byte per element (E4M3 codes): a key row is D bytes = D/128 128-byte chunks.
 template <int D, bool FP8 = false>
 struct MixSmem {
     static constexpr int kHalves = D / 64;                       // 128-byte chunks of a bf16 row (Q tiles, bf16 K / V rows)
     static constexpr int kKvHalves = FP8 ? D / 128 : D / 64;     // 128-byte chunks of a K / V row in the ring
-    static constexpr int kSlot = kHalves * kSlotKeys * 128;      // one K (or V) ring slot
+    static constexpr int kSlot = kKvHalves * kSlotKeys * 128;    // one K (or V) ring slot: 64 keys
+    // Ring depth.  bf16: 5 slots of 16 KB per tensor (4: -1.5 % on pure decode, 6 would not leave room for 2 Q tiles);
+    // a slot then alternates between the two decode warpgroups, so every decode warp takes part in every slot phase.
+    // FP8: 8 slots of 8 KB in less space; with an EVEN ring a slot always belongs to the same decode warpgroup (tile
+    // parity = slot parity), so a warp only touches its own slots - no pass-through waits (kOwnSlots).
+    static constexpr int kNumSt = FP8 ? 8 : 5;
+    static constexpr bool kOwnSlots = kNumSt % 2 == 0;
+    static_assert(kNumSt <= kMaxSt, "barrier index layout");
     // Slot layout = what ONE 4-D TMA box per (page, kv head) slab writes: [8-key group][64-column half][8 rows][128 B],
     // every [8 rows][128 B] block a SWIZZLE_128B core group.  8-key groups are kGroup bytes apart (uniform over the 4
     // pages of a slot: the UMMA stride-byte-offset), the halves of a group 1024 bytes apart.
@@ -98,7 +105,7 @@ struct MixSmem {
     static_assert(kMergeBytes <= kQBytes, "decode merge buffer must fit the Q region");
     static_assert(kQStageOff + kSchedSlots * kQStageBytes <= kQOff + kQBytes, "staged Q blocks must fit beside the merge buffer");
     static constexpr int kBarOff = kQOff + kQBytes;
-    static constexpr int kSchedOff = kBarOff + 512;              // kSchedSlots x 48 B
+    static constexpr int kSchedOff = kBarOff + kBarBytes;        // kSchedSlots x 48 B
     static constexpr int kTmemSlotOff = kSchedOff + kSchedSlots * 48;
     // in-kernel plan (plan.cuh): header + rank tables for up to kPlanMaxR requests, alive for the whole kernel
     static constexpr int kPlanOff = kTmemSlotOff + 32;
@@ -112,13 +119,13 @@ struct MixSmem {
 
 // barrier indices (8 bytes each, from kBarOff)
 enum : int {
-    B_KFULL = 0, B_VFULL = kNumSt, B_KEMPTY_P = 2 * kNumSt, B_KEMPTY_D = 3 * kNumSt, B_VEMPTY_P = 4 * kNumSt,
-    B_VEMPTY_D = 5 * kNumSt,
-    B_SFULL = 6 * kNumSt, B_PFULL = B_SFULL + 4,      // [chain * 2 + buffer]
+    B_KFULL = 0, B_VFULL = kMaxSt, B_KEMPTY_P = 2 * kMaxSt, B_KEMPTY_D = 3 * kMaxSt, B_VEMPTY_P = 4 * kMaxSt,
+    B_VEMPTY_D = 5 * kMaxSt,
+    B_SFULL = 6 * kMaxSt, B_PFULL = B_SFULL + 4,      // [chain * 2 + buffer]
     B_QFULL = B_PFULL + 4, B_QEMPTY = B_QFULL + 1, B_OFULL = B_QEMPTY + 1, B_OFREE = B_OFULL + 2, B_PVDONE = B_OFREE + 2,     // [chain]
     B_SCHED_FULL = B_PVDONE + 2, B_SCHED_EMPTY = B_SCHED_FULL + 4, B_PARTIAL = B_SCHED_EMPTY + 4, B_COUNT = B_PARTIAL + 4
 };
-static_assert(B_COUNT * 8 <= 512, "barrier region");
+static_assert(B_COUNT * 8 <= kBarBytes, "barrier region");
 static_assert(kSchedSlots == 4, "barrier indices assume 4 scheduler slots");
 
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
@@ -278,8 +285,10 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
 #pragma unroll
         for (int mt = 0; mt < D / 16; ++mt) oT[nt][mt][0] = oT[nt][mt][1] = oT[nt][mt][2] = oT[nt][mt][3] = 0.f;
     }
-    // EVERY warp waits FULL and arrives EMPTY on EVERY slot: an mbarrier parity wait is only sound while the waiter is less
-    // than one phase away from the barrier, and with 5 ring slots a slot alternates between the two warpgroups.
+    // Odd ring (bf16, 5 slots): EVERY warp waits FULL and arrives EMPTY on EVERY slot - an mbarrier parity wait is only
+    // sound while the waiter is less than one phase away from the barrier, and a slot alternates between the warpgroups.
+    // Even ring (FP8): tile parity = slot parity, a warp waits and arrives on its own slots only; its barriers see every
+    // one of their decode uses, and a prefill item in between has fully landed before the next item starts (B_QEMPTY).
     const int r16 = cw * kDecKeys;                          // first key row of this warp inside its slots
     const int mi = lane >> 3, l7 = lane & 7;                // ldmatrix: this lane addresses row l7 of matrix mi
 #ifdef SS_PROFILE
@@ -287,10 +296,12 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
 #endif
     for (int t = 0; t < n; ++t) {
         const uint32_t tc = tile_ctr + t;
-        const int s = tc % kNumSt;
-        const uint32_t fpar = (tc / kNumSt) & 1;
+        const int s = tc % SM::kNumSt;
+        const uint32_t fpar = (tc / SM::kNumSt) & 1;
         const int key0 = w.kv_begin + t * kSlotKeys;
-        const int nvalid = (t & 1) == wg ? w.kv_end - (key0 + r16) : 0;       // <= 0: nothing for this warp in this slot
+        if (SM::kOwnSlots && (int)(tc & 1) != wg) continue;    // even ring: the slot belongs to the other warpgroup
+        // <= 0: nothing for this warp in this slot (odd ring: the other warpgroup's turn; it still waits and arrives)
+        const int nvalid = (SM::kOwnSlots || (t & 1) == wg) ? w.kv_end - (key0 + r16) : 0;
         const uint32_t kbase = sbase + SM::kKOff + s * SM::kSlot;
         const uint32_t vbase = sbase + SM::kVOff + s * SM::kSlot;
         float sT[NT][4];
@@ -567,7 +578,7 @@ struct TileStreamer {
             int cg[4];                                             // first 8-key group of each (page, kv head) slab
 #pragma unroll
             for (int p = 0; p < 4; ++p) cg[p] = (pg[p] * Hkv + g) * 2;
-            const int s1 = s + 1 == kNumSt ? 0 : s + 1;
+            const int s1 = s + 1 == SM::kNumSt ? 0 : s + 1;
             uint32_t eb1, epar1;
             look(s1, eb1, epar1);                                  // slot s1's history cannot change while tile s is issued
             while (!ok) ok = mbar_try_wait(eb, epar);
@@ -679,13 +690,13 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     if (trace && threadIdx.x == 0) trace[0] = globaltimer_ns();
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kNumSt; ++s) {
+        for (int s = 0; s < SM::kNumSt; ++s) {
             mbar_init(BAR(B_KFULL + s), 1);
             mbar_init(BAR(B_VFULL + s), 1);
             mbar_init(BAR(B_KEMPTY_P + s), 2);               // one commit per chain
-            mbar_init(BAR(B_KEMPTY_D + s), 8);               // every decode warp, every slot
             mbar_init(BAR(B_VEMPTY_P + s), 2);
-            mbar_init(BAR(B_VEMPTY_D + s), 8);
+            mbar_init(BAR(B_KEMPTY_D + s), SM::kOwnSlots ? 4 : 8);   // the owning warpgroup / every decode warp
+            mbar_init(BAR(B_VEMPTY_D + s), SM::kOwnSlots ? 4 : 8);
         }
         for (int b = 0; b < 4; ++b) {
             mbar_init(BAR(B_SFULL + b), 1);
@@ -900,9 +911,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
 #endif
                     auto issue_s = [&](int kt) {
                         const uint32_t tc = tile_ctr + kt, sc = s_ctr + kt;
-                        const int s = tc % kNumSt, b = sc & 1;
+                        const int s = tc % SM::kNumSt, b = sc & 1;
                         SS_MM(2)
-                        mbar_wait(BAR(B_KFULL + s), (tc / kNumSt) & 1);
+                        mbar_wait(BAR(B_KFULL + s), (tc / SM::kNumSt) & 1);
                         tc_fence_after();
                         SS_MM(1)
                         const uint64_t qdesc0 = umma_desc_sw128(sbase + SM::kQOff + X * SM::kQTile, 16, 1024);
@@ -919,12 +930,12 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     };
                     auto issue_pv = [&](int kt) {
                         const uint32_t tc = tile_ctr + kt, sc = s_ctr + kt;
-                        const int s = tc % kNumSt, b = sc & 1;
+                        const int s = tc % SM::kNumSt, b = sc & 1;
                         SS_MM(2)
                         mbar_wait(BAR(B_PFULL + X * 2 + b), (sc >> 1) & 1);
                         if (kt == 0) mbar_wait(BAR(B_OFREE + X), (n_chain & 1) ^ 1);     // previous epilogue drained O
                         SS_MM(0)
-                        mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
+                        mbar_wait(BAR(B_VFULL + s), (tc / SM::kNumSt) & 1);
                         tc_fence_after();
                         SS_MM(1)
                         const uint64_t vdesc0 = umma_desc_sw128(sbase + SM::kVOff + s * SM::kSlot, 1024, SM::kGroup);   // halves 1024 apart, 8-key groups kGroup
@@ -1010,7 +1021,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
 #endif
                 for (int kt = 0; kt < n; ++kt) {
                     const uint32_t sc = s_ctr + kt, tc = tile_ctr + kt;
-                    const int b = sc & 1, s = tc % kNumSt;
+                    const int b = sc & 1, s = tc % SM::kNumSt;
                     const int key0 = kt * kSlotKeys;
                     const bool tail = key0 + kSlotKeys > w.kv_end;
                     mbar_wait(BAR(B_SFULL + wg * 2 + b), (sc >> 1) & 1);
@@ -1020,7 +1031,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         // (both chains write the same zeros; each fences before its own P arrive).  After the S wait:
                         // S(kt) done => this item's Q landed => every earlier tile landed (see B_QEMPTY), so the
                         // V wait below is never a phase early.
-                        mbar_wait(BAR(B_VFULL + s), (tc / kNumSt) & 1);
+                        mbar_wait(BAR(B_VFULL + s), (tc / SM::kNumSt) & 1);
                         const uint32_t vaddr = sbase + SM::kVOff + s * SM::kSlot;
                         const int first = w.kv_end - key0;
                         for (int i = wtid; i < (kSlotKeys - first) * kHalves * 8; i += 128) {
