@@ -287,8 +287,8 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
     }
     // Odd ring (bf16, 5 slots): EVERY warp waits FULL and arrives EMPTY on EVERY slot - an mbarrier parity wait is only
     // sound while the waiter is less than one phase away from the barrier, and a slot alternates between the warpgroups.
-    // Even ring (FP8): tile parity = slot parity, a warp waits and arrives on its own slots only; its barriers see every
-    // one of their decode uses, and a prefill item in between has fully landed before the next item starts (B_QEMPTY).
+    // Even ring (FP8): every item covers an even number of ring tiles, so item-local tile parity = slot parity and a slot
+    // always belongs to the same warpgroup: a warp waits and arrives on its own slots only, and sees every use of them.
     const int r16 = cw * kDecKeys;                          // first key row of this warp inside its slots
     const int mi = lane >> 3, l7 = lane & 7;                // ldmatrix: this lane addresses row l7 of matrix mi
 #ifdef SS_PROFILE
@@ -299,7 +299,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
         const int s = tc % SM::kNumSt;
         const uint32_t fpar = (tc / SM::kNumSt) & 1;
         const int key0 = w.kv_begin + t * kSlotKeys;
-        if (SM::kOwnSlots && (int)(tc & 1) != wg) continue;    // even ring: the slot belongs to the other warpgroup
+        if (SM::kOwnSlots && (t & 1) != wg) continue;          // even ring: the slot belongs to the other warpgroup
         // <= 0: nothing for this warp in this slot (odd ring: the other warpgroup's turn; it still waits and arrives)
         const int nvalid = (SM::kOwnSlots || (t & 1) == wg) ? w.kv_end - (key0 + r16) : 0;
         const uint32_t kbase = sbase + SM::kKOff + s * SM::kSlot;
@@ -571,8 +571,10 @@ struct TileStreamer {
         };
         int pg1[4];
         load_pages(w.kv_begin + kSlotKeys, pg1);
-        for (int key0 = w.kv_begin; key0 < w.kv_end; key0 += kSlotKeys) {
-            if (key0 + kSlotKeys >= w.kv_end) on_last();
+        const int ntiles = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
+        const int nring = SM::kOwnSlots ? (ntiles + 1) & ~1 : ntiles;      // even ring: pad with an empty tile (see the consumers)
+        for (int i = 0, key0 = w.kv_begin; i < nring; ++i, key0 += kSlotKeys) {
+            if (i == ntiles - 1) on_last();
             int pg2[4];
             load_pages(key0 + 2 * kSlotKeys, pg2);                 // used two iterations from now
             int cg[4];                                             // first 8-key group of each (page, kv head) slab
@@ -590,7 +592,7 @@ struct TileStreamer {
 #pragma unroll
                 for (int p = 0; p < 4; ++p) tma_load_slab(dst + p * SM::kPageBytes, tmap, cg[p], full);
             } else {
-                const int npages = (nkeys + kPage - 1) / kPage;
+                const int npages = nkeys > 0 ? (nkeys + kPage - 1) / kPage : 0;      // 0: the padding tile, a plain arrival
                 mbar_arrive_expect_tx(full, (uint32_t)npages * SM::kPageBytes);
 #pragma unroll
                 for (int p = 0; p < 4; ++p)
@@ -899,7 +901,11 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
             const ss_work_item w = sched[slot];
             const int kind = w.kind;
-            const int n = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
+            // ring tiles of the item; on an even ring (FP8) padded to an even count with an empty tile, so that every
+            // item starts on an even slot and tile parity = slot parity holds with ITEM-LOCAL tile indices (the split of
+            // keys between the warpgroups, hence the summation order, must not depend on what the CTA ran before)
+            const int n = SM::kOwnSlots ? ((w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys + 1) & ~1
+                                        : (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
             ++n_sched;
             if (kind == 0) break;
             if (!FP8 && kind == 1) {
@@ -1003,7 +1009,11 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             const ss_work_item w = sched[slot];
             ++n_sched;
             if (w.kind == 0) break;
-            const int n = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
+            // ring tiles of the item; on an even ring (FP8) padded to an even count with an empty tile, so that every
+            // item starts on an even slot and tile parity = slot parity holds with ITEM-LOCAL tile indices (the split of
+            // keys between the warpgroups, hence the summation order, must not depend on what the CTA ran before)
+            const int n = SM::kOwnSlots ? ((w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys + 1) & ~1
+                                        : (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
             unsigned long long* const tr = (trace && wg == 0 && wtid == 0 && 6 + 9 * (int)n_sched <= prm.trace_words) ? trace + 6 + 9 * (n_sched - 1) : nullptr;
             if (tr) {
                 tr[0] = globaltimer_ns();

@@ -219,3 +219,19 @@ def test_fp8_needs_scales_and_head_dim_128():
     with pytest.raises(binding.SlidingAttnError) as ei:
         binding.handle_for(b64, t64, fp8_caches=(kc64, kc64.clone()))
     assert ei.value.status == binding.SS_ERR_INVALID_ARG
+
+
+def test_fp8_bitwise_reproducible_whatever_ran_before():
+    """The split of an item's keys between the decode warpgroups must not depend on the CTA's history (dynamic queue):
+    repeated calls, and the same batch after a different batch on the same handle, give identical bits."""
+    b = wl.config_c3(0, 1, 128)
+    t = wl.make_tensors(b, DEV, caches=False)
+    kc, vc, ks, vs = wl.make_fp8_caches(b, DEV)
+    h = binding.handle_for(b, t, fp8_caches=(kc, vc), kv_scales=(ks, vs))
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    outs = [binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale).clone() for _ in range(4)]
+    ctx2 = torch.clamp(ctx - 37, min=0)                       # another batch in between: other tile counts per item
+    binding.mixed_attention(h, t.q, bt, qsl, ctx2, b.scale)
+    outs.append(binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale).clone())
+    torch.cuda.synchronize()
+    assert all(torch.equal(outs[0], o) for o in outs[1:])
