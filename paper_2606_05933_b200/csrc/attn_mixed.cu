@@ -574,7 +574,7 @@ struct TileStreamer {
         const int ntiles = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
         const int nring = SM::kOwnSlots ? (ntiles + 1) & ~1 : ntiles;      // even ring: pad with an empty tile (see the consumers)
         for (int i = 0, key0 = w.kv_begin; i < nring; ++i, key0 += kSlotKeys) {
-            if (i == ntiles - 1) on_last();
+            if (i == ntiles - 1) on_last();              // (drawing the next ticket 3 or 5 tiles earlier changes nothing)
             int pg2[4];
             load_pages(key0 + 2 * kSlotKeys, pg2);                 // used two iterations from now
             int cg[4];                                             // first 8-key group of each (page, kv head) slab

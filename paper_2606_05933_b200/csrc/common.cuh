@@ -16,7 +16,8 @@ constexpr int kPage = 16;             // tokens per KV page (BASELINE.json confi
 constexpr int kTileKeys = 128;        // keys per staged KV tile / MMA N
 constexpr int kTileRows = 128;        // query rows per prefill tile / MMA M
 constexpr int kMaxGroup = 16;         // max q heads per kv head on the decode path (MMA M = 16)
-constexpr int kDecodeWaves = 3;       // target decode items per SM when choosing the split length
+constexpr int kDecodeWaves = 1;       // target decode items per SM when choosing the split length (a split costs ~2 us of
+                                      // first-tile wait + merge: 3 or 6 per SM over-split every batch with >= 2 units per SM)
 constexpr int kMinSplitKeys = 512;    // never split a decode KV range finer than this
 constexpr int kMaxSplitKeys = 4096;   // never leave a decode item longer than this
 // SM partition model of the two-queue scheduler (measured on B200): bytes/us one SM streams on the

@@ -235,3 +235,13 @@ def test_fp8_bitwise_reproducible_whatever_ran_before():
     outs.append(binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale).clone())
     torch.cuda.synchronize()
     assert all(torch.equal(outs[0], o) for o in outs[1:])
+
+
+def test_fp8_two_launch_route_more_requests_than_the_in_kernel_plan_holds():
+    """R > 256: the stand-alone work-list kernel plans the batch (prefill chunks skipped there too) and the FP8 main
+    kernel reads its items; prefill rows still come from the plain kernel."""
+    rng = np.random.default_rng(81)
+    reqs = [(1, int(u)) for u in rng.integers(1, 700, size=290)] + [(37, 100), (2, 0)]
+    b = wl.make_batch("fp8-r292", 8, 2, 128, reqs, 82, with_append=True)
+    h = fp8_case(b)
+    assert h.last_launch_count() == 3                        # work list + main + plain kernel
