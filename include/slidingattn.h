@@ -96,9 +96,9 @@ int ss_destroy(ss_handle* h);
  *   ss_kv_append       quantises: code = e4m3(x / scale[g]), the quotient an IEEE fp32 division, rounded to nearest
  *                      even, magnitudes above 448 saturate to 448, NaN -> 0x7F.  Bit-exact against that definition.
  *   ss_mixed_attention same definition as the bf16 path with K = decode(code) * k_scale[g], V likewise; bf16 q / out.
- *                      Decode requests (c_r == 1) run on the split-KV tensor-core path over the FP8 tiles (half the HBM
- *                      bytes; q is rounded to fp16 for the products: exact for |q| in [2^-14, 65504], clamped above);
- *                      prefill chunks (c_r > 1) are served by the plain CUDA-core kernel in this version (correct, slow).
+ *                      The staged codes are widened exactly to fp16 and every product runs on fp16 tensor-core operands
+ *                      (decode: half the HBM bytes; prefill chunks: tcgen05 on fp16 copies of the tiles); q is rounded
+ *                      to fp16 for them - exact for |q| in [2^-14, 65504], clamped above - and P is rounded to fp16.
  *   ss_qkv_rope_append returns SS_ERR_NOT_IMPLEMENTED on an FP8 handle.
  */
 int ss_set_kv_scales(ss_handle* h, const float* k_scale_device, const float* v_scale_device);

@@ -313,12 +313,6 @@ int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table,
         SS_CUDA(h, cudaEventRecord(h->ev1, st), "timing event");
         h->timing_valid = 1;
     }
-    if (h->kv_fp8) {
-        // prefill chunks over an FP8 cache: the plain CUDA-core kernel (the main kernel's plan skipped them)
-        SS_CUDA(h, launch_simple_attention(h, q, block_table, query_start_loc, ctx_lens, R, T, scale, out, lse_or_null, st, 1),
-                "simple attention launch (FP8 prefill rows)");
-        ++n;
-    }
     h->last_launches = (two_kernels ? 1 : 0) + n + h->debug_checks;
     return SS_OK;
 }

@@ -57,7 +57,7 @@ using namespace ptx;
 constexpr int kMixThreads = 384;
 constexpr int kSlotKeys = 64;        // keys per K / V ring slot = keys per S buffer
 constexpr int kMaxSt = 8;            // most K / V ring slots of any instantiation (barrier index layout)
-constexpr int kBarBytes = 640;       // mbarrier block (8 bytes each)
+constexpr int kBarBytes = 704;       // mbarrier block (8 bytes each)
 constexpr int kSchedSlots = 4;
 constexpr int kDecKeys = 16;         // keys of a 64-key slot one decode warp owns (4 warps per slot)
 // setmaxnreg moves registers inside the CTA's own launch allocation: 384 threads x 168 (the __launch_bounds__ cap ptxas
@@ -77,9 +77,10 @@ struct MixSmem {
     static constexpr int kSlot = kKvHalves * kSlotKeys * 128;    // one K (or V) ring slot: 64 keys
     // Ring depth.  bf16: 5 slots of 16 KB per tensor (4: -1.5 % on pure decode, 6 would not leave room for 2 Q tiles);
     // a slot then alternates between the two decode warpgroups, so every decode warp takes part in every slot phase.
-    // FP8: 8 slots of 8 KB in less space; with an EVEN ring a slot always belongs to the same decode warpgroup (tile
-    // parity = slot parity), so a warp only touches its own slots - no pass-through waits (kOwnSlots).
-    static constexpr int kNumSt = FP8 ? 8 : 5;
+    // FP8: 6 slots of 8 KB; with an EVEN ring a slot always belongs to the same decode warpgroup (tile parity = slot
+    // parity), so a warp only touches its own slots - no pass-through waits (kOwnSlots).  The space saved holds the
+    // fp16 copies of the K / V tiles the tensor-core prefill path works on (kConv*, see the converter warps).
+    static constexpr int kNumSt = FP8 ? 6 : 5;
     static constexpr bool kOwnSlots = kNumSt % 2 == 0;
     static_assert(kNumSt <= kMaxSt, "barrier index layout");
     // Slot layout = what ONE 4-D TMA box per (page, kv head) slab writes: [8-key group][64-column half][8 rows][128 B],
@@ -104,7 +105,15 @@ struct MixSmem {
     static constexpr int kQStageBytes = 8 * D * 2;
     static_assert(kMergeBytes <= kQBytes, "decode merge buffer must fit the Q region");
     static_assert(kQStageOff + kSchedSlots * kQStageBytes <= kQOff + kQBytes, "staged Q blocks must fit beside the merge buffer");
-    static constexpr int kBarOff = kQOff + kQBytes;
+    // FP8 prefill: two fp16 K tiles and two fp16 V tiles (64 keys x D) in the bf16 slot layout (8-key groups kConvGroup apart)
+    static constexpr int kConvTile = FP8 ? kHalves * kSlotKeys * 128 : 0;
+    static constexpr int kConvGroup = kHalves * 1024;
+    static constexpr int kKConvOff = kQOff + kQBytes;
+    static constexpr int kVConvOff = kKConvOff + 2 * kConvTile;
+    __device__ static __forceinline__ uint32_t conv_off(int r, int cd) {      // 16-byte chunk cd (0 .. D/8-1) of key row r
+        return (uint32_t)((r >> 3) * kConvGroup + (cd >> 3) * 1024 + (r & 7) * 128 + (((cd & 7) ^ (r & 7)) << 4));
+    }
+    static constexpr int kBarOff = kVConvOff + 2 * kConvTile;
     static constexpr int kSchedOff = kBarOff + kBarBytes;        // kSchedSlots x 48 B
     static constexpr int kTmemSlotOff = kSchedOff + kSchedSlots * 48;
     // in-kernel plan (plan.cuh): header + rank tables for up to kPlanMaxR requests, alive for the whole kernel
@@ -123,7 +132,10 @@ enum : int {
     B_VEMPTY_D = 5 * kMaxSt,
     B_SFULL = 6 * kMaxSt, B_PFULL = B_SFULL + 4,      // [chain * 2 + buffer]
     B_QFULL = B_PFULL + 4, B_QEMPTY = B_QFULL + 1, B_OFULL = B_QEMPTY + 1, B_OFREE = B_OFULL + 2, B_PVDONE = B_OFREE + 2,     // [chain]
-    B_SCHED_FULL = B_PVDONE + 2, B_SCHED_EMPTY = B_SCHED_FULL + 4, B_PARTIAL = B_SCHED_EMPTY + 4, B_COUNT = B_PARTIAL + 4
+    B_SCHED_FULL = B_PVDONE + 2, B_SCHED_EMPTY = B_SCHED_FULL + 4, B_PARTIAL = B_SCHED_EMPTY + 4,
+    // FP8 prefill: fp16 copies of the staged tiles [buffer], and the Q tile converted in place
+    B_KCONV_FULL = B_PARTIAL + 4, B_KCONV_EMPTY = B_KCONV_FULL + 2, B_VCONV_FULL = B_KCONV_EMPTY + 2,
+    B_VCONV_EMPTY = B_VCONV_FULL + 2, B_QCONV = B_VCONV_EMPTY + 2, B_COUNT = B_QCONV + 1
 };
 static_assert(B_COUNT * 8 <= kBarBytes, "barrier region");
 static_assert(kSchedSlots == 4, "barrier indices assume 4 scheduler slots");
@@ -136,6 +148,10 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo
     d |= (uint64_t)1 << 46;                 // descriptor version (Blackwell)
     d |= (uint64_t)2 << 61;                 // layout type: SWIZZLE_128B
     return d;
+}
+// kind::f16 with fp16 A and B operands (FP8 cache: the staged tiles are widened to fp16), fp32 accumulate
+__host__ __device__ constexpr uint32_t umma_idesc_f16(int M, int N, int b_mn_major) {
+    return (1u << 4) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 __host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N, int b_mn_major) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) |
@@ -189,7 +205,7 @@ constexpr int kPolyEvery = SS_POLY_EVERY;      // every kPolyEvery-th pair of sc
 // One 64-key half tile of one query row: S (64 fp32 scores in sr) -> P (bf16 pairs in pk), online-softmax state (m, l).
 // MASKED: keys at and after nvis are invisible (causal diagonal / end of the KV range); replaced by select.
 // Returns alpha (the factor the accumulated O row must be scaled by; 1 unless the reference max moved).
-template <bool MASKED>
+template <bool MASKED, bool F16 = false>
 __device__ __forceinline__ float softmax_half(uint32_t (&sr)[2][32], int nvis, float sl2, float& m, float& l, uint32_t (&pk)[32]) {
     float bm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
@@ -212,7 +228,7 @@ __device__ __forceinline__ float softmax_half(uint32_t (&sr)[2][32], int nvis, f
         const float2 x = __ffma2_rn(make_float2(__uint_as_float(sr[i >> 4][(2 * i) & 31]), __uint_as_float(sr[i >> 4][((2 * i) & 31) + 1])), sl2v, nm);
         const float2 p = (kPolyEvery > 0 && i % (kPolyEvery > 0 ? kPolyEvery : 1) == 0) ? exp2_poly2(x) : make_float2(exp2f(x.x), exp2f(x.y));
         ps[i & 3] = __fadd2_rn(ps[i & 3], p);
-        pk[i] = pack_bf16(p.x, p.y);
+        pk[i] = F16 ? pack_f16(p.x, p.y) : pack_bf16(p.x, p.y);      // FP8 cache: V is widened to fp16, so is P
     }
     const float2 s01 = __fadd2_rn(__fadd2_rn(ps[0], ps[1]), __fadd2_rn(ps[2], ps[3]));
     l = l * alpha + (s01.x + s01.y);
@@ -695,8 +711,8 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         for (int s = 0; s < SM::kNumSt; ++s) {
             mbar_init(BAR(B_KFULL + s), 1);
             mbar_init(BAR(B_VFULL + s), 1);
-            mbar_init(BAR(B_KEMPTY_P + s), 2);               // one commit per chain
-            mbar_init(BAR(B_VEMPTY_P + s), 2);
+            mbar_init(BAR(B_KEMPTY_P + s), FP8 ? 1 : 2);     // one commit per chain; FP8: the K converter pair
+            mbar_init(BAR(B_VEMPTY_P + s), FP8 ? 1 : 2);
             mbar_init(BAR(B_KEMPTY_D + s), SM::kOwnSlots ? 4 : 8);   // the owning warpgroup / every decode warp
             mbar_init(BAR(B_VEMPTY_D + s), SM::kOwnSlots ? 4 : 8);
         }
@@ -706,6 +722,15 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         }
         mbar_init(BAR(B_QFULL), 1);
         mbar_init(BAR(B_QEMPTY), 2);
+        if (FP8) {
+            for (int b = 0; b < 2; ++b) {
+                mbar_init(BAR(B_KCONV_FULL + b), 1);
+                mbar_init(BAR(B_KCONV_EMPTY + b), 1);
+                mbar_init(BAR(B_VCONV_FULL + b), 1);
+                mbar_init(BAR(B_VCONV_EMPTY + b), 1);
+            }
+            mbar_init(BAR(B_QCONV), 128);
+        }
         for (int x = 0; x < 2; ++x) {
             mbar_init(BAR(B_OFULL + x), 1);
             mbar_init(BAR(B_OFREE + x), 128);
@@ -740,7 +765,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     } else if (prm.self_plan) {
         // a2: every CTA builds the same plan (scratch = the still unused K ring); items are decoded from queue tickets
         build_plan<kMixThreads, uint16_t>(prm.qsl, prm.ctx_lens, prm.R, Hq, Hkv, D, prm.num_sms, prm.force_split_keys,
-                                          prm.force_decode_ctas, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph, FP8 ? 1 : 0);
+                                          prm.force_decode_ctas, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph, FP8 ? 1 : 0);   // FP8: single-head prefill items
         fence_proxy_async();    // scratch was written through the generic proxy; TMA writes the same bytes next
     } else if (threadIdx.x == 0) {
         ph->tot_p = prm.hdr->n_prefill;
@@ -891,11 +916,14 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         // for both chains.  The chains touch disjoint TMEM and only read the shared K/V slots, so no order is needed
         // between them; the slot / Q-tile release barriers take one commit per chain (chain A commits twice when the
         // item has a single head).  Decode items: warp 1 has nothing to do, warp 2 runs a5 (split_merge).
-        constexpr uint32_t idesc_qk = umma_idesc_bf16(kTileRows, kSlotKeys, 0);
-        constexpr uint32_t idesc_pv = umma_idesc_bf16(kTileRows, D, 1);
+        // FP8 cache: prefill items have one head (chain A); the operands are the fp16 copies the converter warps (WG2) write
+        // into two K and two V buffers, Q converted in place by chain A's workers; tiles are counted by cv_ctr.
+        constexpr uint32_t idesc_qk = FP8 ? umma_idesc_f16(kTileRows, kSlotKeys, 0) : umma_idesc_bf16(kTileRows, kSlotKeys, 0);
+        constexpr uint32_t idesc_pv = FP8 ? umma_idesc_f16(kTileRows, D, 1) : umma_idesc_bf16(kTileRows, D, 1);
         const int X = warp - 1;
         const uint32_t tchain = tmem_base + X * SM::kTmemChain;
         uint32_t tile_ctr = 0, n_sched = 0, n_pre = 0, s_ctr = 0, n_chain = 0;   // s_ctr / n_chain: this chain's half tiles / items
+        uint32_t cv_ctr = 0;                                                      // FP8: prefill tiles converted so far
         for (;;) {
             const int slot = n_sched % kSchedSlots;
             mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
@@ -906,9 +934,10 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             // keys between the warpgroups, hence the summation order, must not depend on what the CTA ran before)
             const int n = SM::kOwnSlots ? ((w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys + 1) & ~1
                                         : (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;
+            const int nr = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;      // real tiles (n may hold a padding tile)
             ++n_sched;
             if (kind == 0) break;
-            if (!FP8 && kind == 1) {
+            if (kind == 1) {
                 const int nq = w.nheads;
                 if (X < nq && elect_one()) {
                     const int ncommit = nq == 1 ? 2 : 1;          // arrivals this chain owes the shared (count 2) barriers
@@ -918,12 +947,15 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     auto issue_s = [&](int kt) {
                         const uint32_t tc = tile_ctr + kt, sc = s_ctr + kt;
                         const int s = tc % SM::kNumSt, b = sc & 1;
+                        const uint32_t cv = cv_ctr + kt, cb = cv & 1;
                         SS_MM(2)
-                        mbar_wait(BAR(B_KFULL + s), (tc / SM::kNumSt) & 1);
+                        if (FP8) mbar_wait(BAR(B_KCONV_FULL + cb), (cv >> 1) & 1);
+                        else mbar_wait(BAR(B_KFULL + s), (tc / SM::kNumSt) & 1);
                         tc_fence_after();
                         SS_MM(1)
                         const uint64_t qdesc0 = umma_desc_sw128(sbase + SM::kQOff + X * SM::kQTile, 16, 1024);
-                        const uint64_t kdesc0 = umma_desc_sw128(sbase + SM::kKOff + s * SM::kSlot, 16, SM::kGroup);
+                        const uint64_t kdesc0 = FP8 ? umma_desc_sw128(sbase + SM::kKConvOff + cb * SM::kConvTile, 16, SM::kConvGroup)
+                                                    : umma_desc_sw128(sbase + SM::kKOff + s * SM::kSlot, 16, SM::kGroup);
 #pragma unroll
                         for (int ks = 0; ks < D / 16; ++ks) {
                             // bytes; descriptor address unit = 16 B.  64-column halves: Q 128 rows, K 64 rows apart
@@ -932,7 +964,8 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                             umma_ss(tchain + b * 64, qdesc0 + (qoff >> 4), kdesc0 + (koff >> 4), idesc_qk, ks > 0);
                         }
                         umma_commit(BAR(B_SFULL + X * 2 + b));
-                        for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_KEMPTY_P + s));
+                        if (FP8) umma_commit(BAR(B_KCONV_EMPTY + cb));
+                        else for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_KEMPTY_P + s));
                     };
                     auto issue_pv = [&](int kt) {
                         const uint32_t tc = tile_ctr + kt, sc = s_ctr + kt;
@@ -940,17 +973,23 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         SS_MM(2)
                         mbar_wait(BAR(B_PFULL + X * 2 + b), (sc >> 1) & 1);
                         if (kt == 0) mbar_wait(BAR(B_OFREE + X), (n_chain & 1) ^ 1);     // previous epilogue drained O
+                        const uint32_t cv = cv_ctr + kt, cb = cv & 1;
                         SS_MM(0)
-                        mbar_wait(BAR(B_VFULL + s), (tc / SM::kNumSt) & 1);
+                        if (FP8) mbar_wait(BAR(B_VCONV_FULL + cb), (cv >> 1) & 1);
+                        else mbar_wait(BAR(B_VFULL + s), (tc / SM::kNumSt) & 1);
                         tc_fence_after();
                         SS_MM(1)
-                        const uint64_t vdesc0 = umma_desc_sw128(sbase + SM::kVOff + s * SM::kSlot, 1024, SM::kGroup);   // halves 1024 apart, 8-key groups kGroup
+                        // halves 1024 apart, 8-key groups kGroup; 16 keys (one k-step) = two groups
+                        const uint64_t vdesc0 = FP8 ? umma_desc_sw128(sbase + SM::kVConvOff + cb * SM::kConvTile, 1024, SM::kConvGroup)
+                                                    : umma_desc_sw128(sbase + SM::kVOff + s * SM::kSlot, 1024, SM::kGroup);
+                        constexpr uint32_t kstep = 2 * (FP8 ? SM::kConvGroup : SM::kGroup);
 #pragma unroll
                         for (int kk = 0; kk < kSlotKeys / 16; ++kk)      // A = P[b] from TMEM: 16 keys = 8 packed columns
-                            umma_ts(tchain + SM::kTmemO, tchain + b * 64 + kk * 8, vdesc0 + (uint64_t)(kk * SM::kPageBytes >> 4), idesc_pv, (kt > 0 || kk > 0));
+                            umma_ts(tchain + SM::kTmemO, tchain + b * 64 + kk * 8, vdesc0 + (uint64_t)(kk * kstep >> 4), idesc_pv, (kt > 0 || kk > 0));
                         umma_commit(BAR(B_PVDONE + X));
-                        for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_VEMPTY_P + s));
-                        if (kt == n - 1) {
+                        if (FP8) umma_commit(BAR(B_VCONV_EMPTY + cb));
+                        else for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_VEMPTY_P + s));
+                        if (kt == nr - 1) {
                             umma_commit(BAR(B_OFULL + X));
                             // Q tiles free for the next item.  Committed after the LAST MMA of the item (not the last
                             // S): when the next Q tile lands, every K and V tile issued before it has landed too, so a
@@ -960,13 +999,14 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         }
                     };
                     mbar_wait(BAR(B_QFULL), n_pre & 1);
+                    if (FP8) { mbar_wait(BAR(B_QCONV), n_pre & 1); tc_fence_after(); }       // Q tile rewritten as fp16
 #ifdef SS_PROFILE
                     mm_t = clock64();
 #endif
-                    for (int kt = 0; kt < 2 && kt < n; ++kt) issue_s(kt);
-                    for (int kt = 0; kt < n; ++kt) {
+                    for (int kt = 0; kt < 2 && kt < nr; ++kt) issue_s(kt);
+                    for (int kt = 0; kt < nr; ++kt) {
                         issue_pv(kt);
-                        if (kt + 2 < n) issue_s(kt + 2);
+                        if (kt + 2 < nr) issue_s(kt + 2);
                     }
 #ifdef SS_PROFILE
                     SS_MM(2)
@@ -977,7 +1017,8 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
 #endif
                 }
                 __syncwarp();
-                if (X < nq) { s_ctr += n; ++n_chain; }
+                if (X < nq) { s_ctr += nr; ++n_chain; }
+                cv_ctr += nr;
                 ++n_pre;
             } else if (X == 1 && w.nsplit > 1) {
                 split_merge<D>(w, slot, (n_sched - 1) / kSchedSlots, lane, bar0, prm);
@@ -997,10 +1038,11 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         const int row = quarter * 32 + lane;                   // prefill: query row inside the tile
         const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
         const int wtid = threadIdx.x - 128 - wg * 128;         // 0..127 inside the warpgroup
-        const float sl2 = prm.scale * kMLog2e;
+        const float sl2_base = prm.scale * kMLog2e;
         const uint32_t tchain = tmem_base + wg * SM::kTmemChain;
         const uint32_t tmem_o = tchain + SM::kTmemO;
         uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_chain = 0;
+        uint32_t cv_ctr = 0;                                   // FP8 converters (WG2): prefill tiles converted so far
         float* merge = reinterpret_cast<float*>(smem + SM::kQOff);
         if (wg == 0) named_bar_arrive(3, 256);                 // the decode merge buffer starts out free (see stage A below)
         for (;;) {
@@ -1019,8 +1061,23 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 tr[0] = globaltimer_ns();
                 tr[2] = ((unsigned long long)w.kind << 32) | (unsigned)n;
             }
-            if (!FP8 && w.kind == 1 && wg < w.nheads) {
+            const int nr = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;      // real tiles (n may hold a padding tile)
+            if (w.kind == 1 && wg < w.nheads) {
                 // -------------------------- prefill tile, chain wg: thread = query row --------------------------
+                if (FP8) {
+                    // FP8 cache: the MMAs run on fp16 operands - this chain's Q tile is rewritten in place (same swizzled
+                    // positions, bf16 -> fp16: exact for magnitudes in [2^-14, 65504], clamped above) before the first S
+                    mbar_wait(BAR(B_QFULL), n_chain & 1);
+                    uint8_t* qt = smem + SM::kQOff + wg * SM::kQTile;
+                    for (int i = wtid; i < SM::kQTile / 16; i += 128) {
+                        uint4 v = *reinterpret_cast<uint4*>(qt + i * 16);
+                        v.x = bf16x2_to_f16x2(v.x); v.y = bf16x2_to_f16x2(v.y); v.z = bf16x2_to_f16x2(v.z); v.w = bf16x2_to_f16x2(v.w);
+                        *reinterpret_cast<uint4*>(qt + i * 16) = v;
+                    }
+                    fence_proxy_async();
+                    mbar_arrive(BAR(B_QCONV));
+                }
+                const float sl2 = sl2_base * (FP8 ? __ldg(prm.k_scale + w.head / G) : 1.f);
                 const int u = __ldg(prm.ctx_lens + w.req);
                 const int limit = u + w.q_pos0 + row + 1;            // keys [0, limit) visible to this row
                 const int limit_w = u + w.q_pos0 + quarter * 32 + 1;  // ... to the first row of this warp (the fewest)
@@ -1029,14 +1086,14 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
 #ifdef SS_PROFILE
                 long long pf_t = clock64(), pf_acc[4] = {0, 0, 0, 0};     // S wait | tcgen05.ld | softmax | st + fence + arrive
 #endif
-                for (int kt = 0; kt < n; ++kt) {
+                for (int kt = 0; kt < nr; ++kt) {
                     const uint32_t sc = s_ctr + kt, tc = tile_ctr + kt;
                     const int b = sc & 1, s = tc % SM::kNumSt;
                     const int key0 = kt * kSlotKeys;
                     const bool tail = key0 + kSlotKeys > w.kv_end;
                     mbar_wait(BAR(B_SFULL + wg * 2 + b), (sc >> 1) & 1);
                     tc_fence_after();
-                    if (tail) {
+                    if (tail && !FP8) {                          // (FP8: the converter writes zeros for the rows past kv_end)
                         // zero V rows [kv_end - key0, 64): stale / unused-slot bits must not meet P = 0 in the MMA
                         // (both chains write the same zeros; each fences before its own P arrive).  After the S wait:
                         // S(kt) done => this item's Q landed => every earlier tile landed (see B_QEMPTY), so the
@@ -1061,9 +1118,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     uint32_t pk[32];
                     float alpha;
                     if (limit_w - key0 >= kSlotKeys && !tail)       // warp-uniform: every row of this warp sees all 64 keys
-                        alpha = softmax_half<false>(sr, kSlotKeys, sl2, m, l, pk);
+                        alpha = softmax_half<false, FP8>(sr, kSlotKeys, sl2, m, l, pk);
                     else
-                        alpha = softmax_half<true>(sr, min(limit, w.kv_end) - key0, sl2, m, l, pk);
+                        alpha = softmax_half<true, FP8>(sr, min(limit, w.kv_end) - key0, sl2, m, l, pk);
                     SS_PF(2)
                     tmem_st_32x32b_x32(tchain + b * 64 + lane_addr, pk);        // P in place over S
                     if (kt > 0 && !__all_sync(0xffffffffu, alpha == 1.f)) {
@@ -1081,7 +1138,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                     }
                     tmem_st_wait();
                     tc_fence_before();
-                    if (tail) fence_proxy_async();   // zeroed V rows -> visible to the MMA's async proxy
+                    if (tail && !FP8) fence_proxy_async();   // zeroed V rows -> visible to the MMA's async proxy
                     mbar_arrive(BAR(B_PFULL + wg * 2 + b));
                     SS_PF(3)
                 }
@@ -1098,7 +1155,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
 #ifdef SS_PROFILE
                 if (tr) tr[5] = (unsigned long long)pf_acc[0] | ((unsigned long long)(clock64() - pf_t) << 32);
 #endif
-                const float inv = 1.f / l;
+                const float inv = (FP8 ? __ldg(prm.v_scale + w.head / G) : 1.f) / l;
                 const bool store = row < w.nrows;
                 __nv_bfloat16* orow = prm.out + ((int64_t)(w.row0 + row) * Hq + head) * D;
                 // thread = row: D fp32 -> D bf16 = 2 D bytes contiguous, written as 32-byte (whole-sector) stores
@@ -1125,10 +1182,51 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 tc_fence_before();
                 mbar_arrive(BAR(B_OFREE + wg));
                 if (wg == 0) mbar_arrive(BAR(B_PARTIAL + slot));    // keeps the per-slot phase count in step (decode-only use)
-                s_ctr += n;
+                s_ctr += nr;
                 ++n_chain;
             } else if (w.kind == 1) {
-                // single-head item: chain B has nothing to do
+                // single-head item: chain B has nothing to do - except over an FP8 cache, where its four warps widen the
+                // staged tiles to fp16 for the tensor cores: warps 0, 1 the K tiles, warps 2, 3 the V tiles, each pair at
+                // its own pace (K(t) needs S(t-2) done, V(t) needs PV(t-2) done).  A 16-byte chunk of codes becomes two
+                // chunks of the fp16 tile (same swizzled slot layout as a bf16 tile); rows past kv_end are written as
+                // zeros (unused slots may hold NaN codes; 0 * NaN = NaN in the PV product).
+                if (FP8) {
+                    const int is_v = cw >> 1;
+                    const int ct = (cw & 1) * 32 + lane;                                  // 0 .. 63 inside the pair
+                    const uint32_t ring = sbase + (is_v ? SM::kVOff : SM::kKOff);
+                    const uint32_t conv = sbase + (is_v ? SM::kVConvOff : SM::kKConvOff);
+                    const int b_full = is_v ? B_VFULL : B_KFULL, b_empty = is_v ? B_VEMPTY_P : B_KEMPTY_P;
+                    const int c_full = is_v ? B_VCONV_FULL : B_KCONV_FULL, c_empty = is_v ? B_VCONV_EMPTY : B_KCONV_EMPTY;
+                    for (int t = 0; t < n; ++t) {                                         // ring tiles, padding tile included
+                        const uint32_t tc = tile_ctr + t;
+                        const int s = tc % SM::kNumSt;
+                        mbar_wait(BAR(b_full + s), (tc / SM::kNumSt) & 1);
+                        const uint32_t cv = cv_ctr + t, cb = cv & 1;
+                        if (t < nr) {
+                            mbar_wait(BAR(c_empty + cb), ((cv >> 1) & 1) ^ 1);            // the MMAs that read this buffer are done
+                            const int nkeys = w.kv_end - t * kSlotKeys;
+                            const uint32_t src = ring + s * SM::kSlot, dst = conv + cb * SM::kConvTile;
+#pragma unroll 4
+                            for (int q = ct; q < kSlotKeys * 8; q += 64) {
+                                const int r = q >> 3, cd = q & 7;
+                                uint32_t c0 = 0u, c1 = 0u, c2 = 0u, c3 = 0u;
+                                if (r < nkeys)
+                                    asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(c0), "=r"(c1), "=r"(c2), "=r"(c3) : "r"(src + SM::kv_off(r, cd)));
+                                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + SM::conv_off(r, 2 * cd)), "r"(e4m3x2_to_f16x2(c0)),
+                                             "r"(e4m3x2_hi_to_f16x2(c0)), "r"(e4m3x2_to_f16x2(c1)), "r"(e4m3x2_hi_to_f16x2(c1)) : "memory");
+                                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + SM::conv_off(r, 2 * cd + 1)), "r"(e4m3x2_to_f16x2(c2)),
+                                             "r"(e4m3x2_hi_to_f16x2(c2)), "r"(e4m3x2_to_f16x2(c3)), "r"(e4m3x2_hi_to_f16x2(c3)) : "memory");
+                            }
+                            fence_proxy_async();                                          // generic writes -> the MMA's async proxy
+                        }
+                        named_bar_sync(4 + is_v, 64);
+                        if (ct == 0) {
+                            if (t < nr) mbar_arrive(BAR(c_full + cb));
+                            mbar_arrive(BAR(b_empty + s));                                // the ring slot is free
+                        }
+                    }
+                    cv_ctr += nr;
+                }
             } else {
                 // -------------------------- decode split: all 8 worker warps --------------------------
                 // Warp dw owns 16 keys of every other 64-key slot: warps 0-3 (WG1) the even slots of the item, warps 4-7

@@ -238,10 +238,36 @@ def test_fp8_bitwise_reproducible_whatever_ran_before():
 
 
 def test_fp8_two_launch_route_more_requests_than_the_in_kernel_plan_holds():
-    """R > 256: the stand-alone work-list kernel plans the batch (prefill chunks skipped there too) and the FP8 main
-    kernel reads its items; prefill rows still come from the plain kernel."""
+    """R > 256: the stand-alone work-list kernel plans the batch (single-head prefill items) and the FP8 main kernel
+    reads its items."""
     rng = np.random.default_rng(81)
     reqs = [(1, int(u)) for u in rng.integers(1, 700, size=290)] + [(37, 100), (2, 0)]
     b = wl.make_batch("fp8-r292", 8, 2, 128, reqs, 82, with_append=True)
     h = fp8_case(b)
-    assert h.last_launch_count() == 3                        # work list + main + plain kernel
+    assert h.last_launch_count() == 2                        # work list + main
+
+
+def _edge_rows(b, per_req=24, seed=0):
+    """Rows worth checking one by one: first / last of every request and of every 128-row tile, plus a random share."""
+    rng = np.random.default_rng(seed)
+    rows = set()
+    for r, (c, u) in enumerate(b.reqs):
+        s = int(b.query_start_loc[r])
+        for j in {0, c - 1, *range(127, c, 128), *range(128, c, 128), *(int(x) for x in rng.integers(0, max(c, 1), size=min(per_req, c)))}:
+            if 0 <= j < c:
+                rows.add(s + j)
+    return sorted(rows)
+
+
+@pytest.mark.parametrize("reqs,shape", [
+    ([(300, 0), (1, 77)], (8, 2, 128)),                       # 3 row tiles, odd and even ring-tile counts (padding tile)
+    ([(128, 128), (129, 63), (127, 1), (2, 0), (1, 500)], (32, 8, 128)),
+    ([(65, 4031), (64, 64), (1, 4095)], (28, 4, 128)),        # G = 7: odd group, single-head items
+    ([(2048, 4096)], (32, 8, 128)),                           # PP-b
+    ([(1024, 0), (1024, 6000), (1, 3000), (1, 9000)], (64, 8, 128)),   # 70B shape, PP-f + decodes
+])
+def test_fp8_prefill_on_tensor_cores(reqs, shape):
+    """Prefill chunks over the FP8 cache: tcgen05 on fp16 copies of the staged tiles (converter warps), single-head items."""
+    Hq, Hkv, D = shape
+    b = wl.make_batch("fp8-prefill", Hq, Hkv, D, reqs, 90 + len(reqs), with_append=True)
+    fp8_case(b, seed=len(reqs), check_rows=_edge_rows(b) if b.T > 700 else None)
