@@ -31,6 +31,10 @@
 //                 rows (bandwidth-bound, wasted rows are free), online softmax in registers with quad shuffles,
 //                 two-stage cross-warp log-sum-exp merge through smem (WG2 -> WG1 in registers, then 4 -> 1), then
 //                 either the final bf16 row or an fp32 partial.
+//   FP8 cache (template FP8, SS_FLAG_KV_FP8): E4M3 codes through the same TMA boxes on 128-byte rows (6-slot rings).
+//               Decode: codes widened exactly to fp16 after ldmatrix, f16 mma.sync.  Prefill: single-head items; WG2's
+//               warps widen each staged tile into fp16 tiles in the bf16 slot layout for the tcgen05 MMAs (kind::f16 on
+//               fp16 operands), WG1 rewrites the Q tile as fp16 in place.
 // Rooflines: decode items HBM (2*D*2 bytes per cached token per kv head), prefill items bf16 tensor
 // (4*D flop per visible (row,key) pair per head).  V rows at/after kv_end are zeroed in smem before any
 // PV product (unused slots may hold NaN; 0*NaN = NaN); masked scores are replaced, never multiplied.

@@ -116,7 +116,7 @@ def test_rope_theta_must_be_finite_and_above_one():
 
 
 # ------------------------------------------------------------------------------------------------------------------
-# NEXT-3: FP8 E4M3 KV cache (a1 quantising append, a4 decode over FP8 tiles, prefill rows by the plain kernel)
+# NEXT-3: FP8 E4M3 KV cache (a1 quantising append, a4 decode over FP8 tiles, a3 prefill on fp16 copies of the FP8 tiles)
 # ------------------------------------------------------------------------------------------------------------------
 def fp8_scales(Hkv, seed):
     rng = np.random.default_rng(seed)
