@@ -78,10 +78,6 @@ __device__ __forceinline__ void bulk_load_1d(uint32_t dst, const void* src, uint
                  ::"r"(dst), "l"(reinterpret_cast<uint64_t>(src)), "r"(bytes), "r"(bar)
                  : "memory");
 }
-// L2 prefetch of a contiguous global range (16-byte aligned, size multiple of 16): no shared memory, no completion
-__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(reinterpret_cast<uint64_t>(src)), "r"(bytes) : "memory");
-}
 // atomic add with acquire-release semantics at gpu scope: orders this CTA's earlier global writes (made visible to
 // the issuing thread by a CTA barrier) before the add, and later reads after it.
 __device__ __forceinline__ int atom_add_acq_rel_gpu(int32_t* addr, int v) {
@@ -99,12 +95,6 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
     uint32_t v;
     asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr));
     return v;
-}
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* m, int c0, int c1, int c2, uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
-        : "memory");
 }
 
 // ------------------------------------------------------------------ warp-level tensor ops (decode path)
