@@ -102,9 +102,9 @@ struct MixSmem {
     static constexpr int kQOff = kVOff + kNumSt * kSlot;         // 2 Q tiles (prefill) / decode: cross-warp merge buffer + staged Q rows
     static constexpr int kQBytes = 2 * kQTile;
     static constexpr int kMergeBytes = 4 * kMaxGroup * (D + 2) * 4;
-    // decode with G <= 8: merge buffer of 8 rows per warp, then kSchedSlots staged Q blocks (G rows x D bf16, one per
+    // decode with G <= 8: merge buffer of 8 rows per warp (8 warps), then kSchedSlots staged Q blocks (G rows x D bf16, one per
     // scheduler slot, bulk-copied by the producer so the workers never wait on a cold global Q load)
-    static constexpr int kMerge8Bytes = 4 * 8 * (D + 2) * 4;
+    static constexpr int kMerge8Bytes = 8 * 8 * (D + 2) * 4;     // G <= 8: one partial per decode warp, merged 8 -> 1 in one pass
     static constexpr int kQStageOff = kQOff + (kMerge8Bytes + 127) / 128 * 128;
     static constexpr int kQStageBytes = 8 * D * 2;
     static_assert(kMergeBytes <= kQBytes, "decode merge buffer must fit the Q region");
@@ -470,7 +470,9 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
             l[nt][0] += __shfl_xor_sync(0xffffffffu, l[nt][0], o);
             l[nt][1] += __shfl_xor_sync(0xffffffffu, l[nt][1], o);
         }
-    float* mine = merge + cw * mrows * (D + 2);
+    // G <= 8 (NT = 1): every warp writes its partial, one 8 -> 1 pass by all 256 threads.  G > 8: eight 16-row partials
+    // do not fit the buffer - two stages over a 4-warp buffer (WG2 -> WG1 in registers, then 4 -> 1 by WG1).
+    float* mine = merge + (NT == 1 ? wg * 4 + cw : cw) * mrows * (D + 2);
     const int dA = FP8 ? 2 * qr : qr, dB = FP8 ? 2 * qr + 1 : qr + 8;     // d (inside a 16-d block) of accumulator rows qr, qr + 8
     auto put = [&]() {
 #pragma unroll
@@ -490,6 +492,39 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
             }
         }
     };
+    if (NT == 1) {
+        named_bar_sync(2, 256);                   // every thread is done reading the previous decode item's partials
+        put();
+        named_bar_sync(2, 256);
+        if (tr) tr[5] = globaltimer_ns();
+        for (int e = wg * 128 + wtid; e < G * D; e += 256) {
+            const int r = e / D, d = e % D;
+            float M = -INFINITY;
+#pragma unroll
+            for (int x = 0; x < 8; ++x) M = fmaxf(M, merge[(x * mrows + r) * (D + 2) + D]);
+            float L = 0.f, acc = 0.f;
+#pragma unroll
+            for (int x = 0; x < 8; ++x) {
+                const float* src = merge + (x * mrows + r) * (D + 2);
+                const float wgt = exp2f(src[D] - M);           // a warp that saw no key: m = -inf -> weight 0
+                L += src[D + 1] * wgt;
+                acc += src[d] * wgt;
+            }
+            acc *= vs;
+            if (w.nsplit == 1) {
+                const int64_t orow = (int64_t)w.row0 * Hq + (int64_t)w.head * G + r;
+                prm.out[orow * D + d] = __float2bfloat16_rn(acc / L);
+                if (prm.lse && d == 0) prm.lse[orow] = (M + log2f(L)) * kMLn2;
+            } else {
+                float* dst = prm.partials + ((int64_t)(w.partial + w.split) * G + r) * (D + 2);
+                dst[d] = acc;
+                if (d == 0) { dst[D] = M; dst[D + 1] = L; }
+            }
+        }
+        if (tr) tr[6] = globaltimer_ns();
+        mbar_arrive(BAR(B_PARTIAL + slot));       // release (CTA) of this thread's partial stores to the a5 warp; count 256
+        return;
+    }
     if (wg == 1) {
         // stage A: WG2's warp cw hands its partial to WG1's warp cw (same fragment coordinates).  The buffer is free
         // once WG1 has finished the previous decode item's merge (named barrier 3: WG1 arrives, WG2 syncs).
@@ -741,7 +776,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             mbar_init(BAR(B_PVDONE + x), 1);
         }
         for (int s = 0; s < kSchedSlots; ++s) {
-            mbar_init(BAR(B_PARTIAL + s), 128);
+            mbar_init(BAR(B_PARTIAL + s), G <= 8 ? 256 : 128);   // the threads that store decode partials (see decode_item)
             mbar_init(BAR(B_SCHED_FULL + s), 1);
             mbar_init(BAR(B_SCHED_EMPTY + s), 11);               // 2 MMA warps (warp 2 = a5) + the V producer + 8 worker warps
         }
@@ -1048,7 +1083,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_chain = 0;
         uint32_t cv_ctr = 0;                                   // FP8 converters (WG2): prefill tiles converted so far
         float* merge = reinterpret_cast<float*>(smem + SM::kQOff);
-        if (wg == 0) named_bar_arrive(3, 256);                 // the decode merge buffer starts out free (see stage A below)
+        if (wg == 0 && G > 8) named_bar_arrive(3, 256);        // G > 8: the decode merge buffer starts out free (stage A of decode_item)
         for (;;) {
             const int slot = n_sched % kSchedSlots;
             mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
@@ -1185,7 +1220,6 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 if (store && prm.lse) prm.lse[(int64_t)(w.row0 + row) * Hq + head] = (m + log2f(l)) * kMLn2;
                 tc_fence_before();
                 mbar_arrive(BAR(B_OFREE + wg));
-                if (wg == 0) mbar_arrive(BAR(B_PARTIAL + slot));    // keeps the per-slot phase count in step (decode-only use)
                 s_ctr += nr;
                 ++n_chain;
             } else if (w.kind == 1) {
@@ -1237,12 +1271,13 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 // (WG2) the odd ones.  The products are taken TRANSPOSED, keys on the M = 16 side of mma.sync.m16n8k16
                 // and the G query heads of the KV head on the N = 8 side:  S^T = K Q^T  (A = K rows from smem by
                 // ldmatrix, B = Q^T from the staged Q rows),  O^T += V^T P^T  (A = V by ldmatrix.trans, B = P^T by
-                // movmatrix from the S^T accumulators).  With heads padded to M = 16 instead, a 64-key tile cost 128 HMMA
-                // and the legacy tensor path (~1 HMMA.16816 per 9 clk and SM) capped an SM at ~52 GB/s whatever the
-                // ring depth, copy mechanism or warp count (profiles/r2b.md); this form needs 64 (G <= 8).
+                // movmatrix from the S^T accumulators): half the HMMA count and a quarter of the accumulator registers of
+                // padding the heads to M = 16 (64 HMMA per 64-key tile for G <= 8).
                 if (G <= 8) decode_item<D, 1, FP8>(w, n, slot, tile_ctr, wg, cw, lane, wtid, sbase, bar0, prm, merge, tr);
                 else        decode_item<D, 2, FP8>(w, n, slot, tile_ctr, wg, cw, lane, wtid, sbase, bar0, prm, merge, tr);
             }
+            // prefill items: keep B_PARTIAL's per-slot phase count in step (its waiters only look at decode items)
+            if (w.kind == 1 && (G <= 8 || wg == 0)) mbar_arrive(BAR(B_PARTIAL + slot));
             tile_ctr += n;
             if (tr) tr[1] = globaltimer_ns();
             __syncwarp();
