@@ -29,8 +29,8 @@
 //               decode item: all 8 worker warps; a warp owns 16 keys of every other 64-key slot (WG1 the even slots
 //                 of the item, WG2 the odd ones): mma.sync.m16n8k16 with the G query heads of the KV head padded to 16
 //                 rows (bandwidth-bound, wasted rows are free), online softmax in registers with quad shuffles,
-//                 two-stage cross-warp log-sum-exp merge through smem (WG2 -> WG1 in registers, then 4 -> 1), then
-//                 either the final bf16 row or an fp32 partial.
+//                 cross-warp log-sum-exp merge through smem (G <= 8: one 8 -> 1 pass by all 256 threads; G > 8: WG2 ->
+//                 WG1 in registers, then 4 -> 1), then either the final bf16 row or an fp32 partial.
 //   FP8 cache (template FP8, SS_FLAG_KV_FP8): E4M3 codes through the same TMA boxes on 128-byte rows (6-slot rings).
 //               Decode: codes widened exactly to fp16 after ldmatrix, f16 mma.sync.  Prefill: single-head items; WG2's
 //               warps widen each staged tile into fp16 tiles in the bf16 slot layout for the tcgen05 MMAs (kind::f16 on
