@@ -271,3 +271,33 @@ def test_fp8_prefill_on_tensor_cores(reqs, shape):
     Hq, Hkv, D = shape
     b = wl.make_batch("fp8-prefill", Hq, Hkv, D, reqs, 90 + len(reqs), with_append=True)
     fp8_case(b, seed=len(reqs), check_rows=_edge_rows(b) if b.T > 700 else None)
+
+
+def test_randomized_shapes_and_mixes_bf16_and_fp8():
+    """48 seeded random batches over ten layer shapes (G = 1, 2, 3, 4, 7, 8, 16; head_dim 64 and 128), 0-3 prefill chunks and
+    0-39 decodes of random lengths each, alternately over the bf16 and the FP8 cache: append bit-exact, every row against
+    the fp64 oracle."""
+    shapes = [(8, 2, 128), (32, 8, 128), (28, 4, 128), (64, 8, 128), (16, 1, 128), (4, 4, 64), (16, 4, 64), (8, 8, 64),
+              (14, 2, 128), (12, 4, 128)]
+    rng = np.random.default_rng(12345)
+    for it in range(48):
+        Hq, Hkv, D = shapes[it % len(shapes)]
+        npf, nd = int(rng.integers(0, 4)), int(rng.integers(0, 40))
+        nd = max(nd, 1 if npf == 0 else 0)
+        b = wl.random_batch(70000 + it, Hq=Hq, Hkv=Hkv, D=D, n_prefill=npf, n_decode=nd, max_c=int(rng.integers(2, 400)),
+                            max_u=int(rng.integers(1, 5000)))
+        b = wl.Batch(**{**b.__dict__, "with_append": True})
+        if D == 128 and it % 2 == 1:
+            fp8_case(b, seed=it)
+            continue
+        t = wl.make_tensors(b, DEV, poison_unused=True)
+        k0, v0 = wl.to_u16(t.k_cache), wl.to_u16(t.v_cache)
+        h = binding.handle_for(b, t)
+        bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+        binding.kv_append(h, t.k_new, t.v_new, bt, qsl, ctx)
+        out = binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale)
+        torch.cuda.synchronize()
+        oracle.kv_append(k0, v0, wl.to_u16(t.k_new), wl.to_u16(t.v_new), b.block_table, b.query_start_loc, b.ctx_lens)
+        assert np.array_equal(wl.to_u16(t.k_cache), k0) and np.array_equal(wl.to_u16(t.v_cache), v0)
+        ref, _, _ = oracle.mixed_attention(wl.to_u16(t.q), k0, v0, b.block_table, b.query_start_loc, b.ctx_lens, b.scale)
+        check_attention(b, out, ref)
