@@ -85,7 +85,7 @@ struct Handle {
 inline WorkspaceLayout workspace_layout(const ss_config& c, int num_sms) {
     WorkspaceLayout w{};
     const int64_t group = c.num_q_heads / c.num_kv_heads;
-    const int64_t tiles = (int64_t)(c.max_tokens + kTileRows - 1) / kTileRows + c.max_requests;
+    const int64_t tiles = ((int64_t)c.max_tokens + kTileRows - 1) / kTileRows + c.max_requests;   // widen BEFORE the add
     const int64_t max_prefill = (int64_t)c.num_q_heads * tiles;
     // decode items: Hkv * sum_r nsplit_r.  Unclamped split length: <= Hkv*R + num_sms*kDecodeWaves;
     // split length clamped at kMaxSplitKeys: <= Hkv * R * (ceil(max ctx / kMaxSplitKeys) + 1).
