@@ -99,7 +99,7 @@ int ss_destroy(ss_handle* h);
  *                      The staged codes are widened exactly to fp16 and every product runs on fp16 tensor-core operands
  *                      (decode: half the HBM bytes; prefill chunks: tcgen05 on fp16 copies of the tiles); q is rounded
  *                      to fp16 for them - exact for |q| in [2^-14, 65504], clamped above - and P is rounded to fp16.
- *   ss_qkv_rope_append returns SS_ERR_NOT_IMPLEMENTED on an FP8 handle.
+ *   ss_qkv_rope_append rotates as on a bf16 handle (k rounded to bf16 once), then quantises k and v exactly as ss_kv_append does.
  */
 int ss_set_kv_scales(ss_handle* h, const float* k_scale_device, const float* v_scale_device);
 

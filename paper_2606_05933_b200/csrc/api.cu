@@ -270,7 +270,7 @@ int ss_qkv_rope_append(ss_handle* hh, const void* qkv, const int32_t* block_tabl
     if (R == 0 || T == 0) return SS_OK;
     if (!block_table || (((uintptr_t)block_table) & 3u)) return SS_ERR_INVALID_ARG;
     if (!(rope_theta > 1.f) || !isfinite(rope_theta)) return SS_ERR_INVALID_ARG;
-    if (h->kv_fp8) return SS_ERR_NOT_IMPLEMENTED;
+    if (h->kv_fp8 && !h->k_scale) return SS_ERR_INVALID_ARG;          // ss_set_kv_scales first
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (h->debug_checks) SS_CUDA(h, launch_validate(h, block_table, query_start_loc, ctx_lens, R, T, st), "validate launch");
     SS_CUDA(h, launch_qkv_rope_append(h, qkv, block_table, query_start_loc, ctx_lens, R, T, rope_theta, q_out, st),

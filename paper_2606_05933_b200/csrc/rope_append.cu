@@ -19,9 +19,19 @@ __device__ __forceinline__ float2 bf2_to_f2(uint32_t w) {
     return make_float2(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u));
 }
 
+// two bf16 (one word) -> two E4M3 codes: exact widening, IEEE fp32 division by the head's scale, RNE with saturation -
+// the quantisation of kv_append_fp8_kernel applied to the bf16 value the bf16 path would have stored
+__device__ __forceinline__ uint32_t bf16x2_to_e4m3x2(uint32_t w, float sc) {
+    return ptx::f32x2_to_e4m3x2(ptx::div_rn_ieee(__uint_as_float(w << 16), sc), ptx::div_rn_ieee(__uint_as_float(w & 0xffff0000u), sc));
+}
+
+// FP8 (SS_FLAG_KV_FP8): q as before; the rotated k is rounded to bf16 exactly as on the bf16 path and THEN quantised like
+// ss_kv_append does (so is v): the caches are byte arrays, k_cache / v_cache are passed as their byte addresses.
+template <bool FP8>
 __global__ void __launch_bounds__(kRopeThreads)
 qkv_rope_append_kernel(const uint32_t* __restrict__ qkv, uint32_t* __restrict__ q_out, uint32_t* __restrict__ k_cache,
-                       uint4* __restrict__ v_cache, const int32_t* __restrict__ block_table,
+                       uint4* __restrict__ v_cache, const float* __restrict__ k_scale, const float* __restrict__ v_scale,
+                       const int32_t* __restrict__ block_table,
                        const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int max_pages,
                        int Hq, int Hkv, int D, double neg2_log2_theta_over_d, const int32_t* __restrict__ err_flag) {
     __shared__ float s_cos[64], s_sin[64];
@@ -53,6 +63,14 @@ qkv_rope_append_kernel(const uint32_t* __restrict__ qkv, uint32_t* __restrict__ 
         const float c0 = s_cos[2 * w], c1 = s_cos[2 * w + 1], s0 = s_sin[2 * w], s1 = s_sin[2 * w + 1];
         const uint32_t ylo = ptx::pack_bf16(__fmaf_rn(a.x, c0, -(b.x * s0)), __fmaf_rn(a.y, c1, -(b.y * s1)));
         const uint32_t yhi = ptx::pack_bf16(__fmaf_rn(b.x, c0, a.x * s0), __fmaf_rn(b.y, c1, a.y * s1));
+        if (FP8 && h >= Hq) {
+            const int g = h - Hq;
+            const float sc = __ldg(k_scale + g);
+            uint16_t* kd = reinterpret_cast<uint16_t*>(reinterpret_cast<uint8_t*>(k_cache) + ((page * Hkv + g) * kPage + slot) * (int64_t)D);
+            kd[w] = (uint16_t)bf16x2_to_e4m3x2(ylo, sc);                 // elements 2w, 2w + 1
+            kd[hw + w] = (uint16_t)bf16x2_to_e4m3x2(yhi, sc);            // elements D/2 + 2w, + 1
+            continue;
+        }
         uint32_t* dst = h < Hq ? q_out + ((int64_t)tok * Hq + h) * wpr
                                : k_cache + ((page * Hkv + (h - Hq)) * kPage + slot) * (int64_t)wpr;
         dst[w] = ylo;
@@ -63,7 +81,15 @@ qkv_rope_append_kernel(const uint32_t* __restrict__ qkv, uint32_t* __restrict__ 
     const uint4* vsrc = reinterpret_cast<const uint4*>(src + (Hq + Hkv) * wpr);
     for (int e = tid; e < Hkv * vph; e += kRopeThreads) {
         const int g = e / vph, dv = e - g * vph;
-        v_cache[((page * Hkv + g) * kPage + slot) * (int64_t)vph + dv] = __ldg(vsrc + e);
+        const uint4 v = __ldg(vsrc + e);
+        if (FP8) {
+            const float sc = __ldg(v_scale + g);
+            uint2* vd = reinterpret_cast<uint2*>(reinterpret_cast<uint8_t*>(v_cache) + ((page * Hkv + g) * kPage + slot) * (int64_t)D);
+            vd[dv] = make_uint2(bf16x2_to_e4m3x2(v.x, sc) | (bf16x2_to_e4m3x2(v.y, sc) << 16),
+                                bf16x2_to_e4m3x2(v.z, sc) | (bf16x2_to_e4m3x2(v.w, sc) << 16));
+        } else {
+            v_cache[((page * Hkv + g) * kPage + slot) * (int64_t)vph + dv] = v;
+        }
     }
 }
 
@@ -71,10 +97,14 @@ cudaError_t launch_qkv_rope_append(const Handle* h, const void* qkv, const int32
                                    const int32_t* ctx, int R, int T, float rope_theta, void* q_out, cudaStream_t stream) {
     const ss_config& c = h->cfg;
     const double k = -2.0 * log2((double)rope_theta) / (double)c.head_dim;
-    return launch_pdl(qkv_rope_append_kernel, dim3((unsigned)T), dim3(kRopeThreads), 0, stream, (const uint32_t*)qkv,
-                      (uint32_t*)q_out, (uint32_t*)h->k_cache, (uint4*)h->v_cache, bt, qsl, ctx, R, c.max_pages_per_req,
-                      c.num_q_heads, c.num_kv_heads, c.head_dim, k,
-                      (const int32_t*)(h->debug_checks ? h->state + kStateErr : nullptr));
+    const int32_t* flag = h->debug_checks ? h->state + kStateErr : nullptr;
+    if (h->kv_fp8)
+        return launch_pdl(qkv_rope_append_kernel<true>, dim3((unsigned)T), dim3(kRopeThreads), 0, stream, (const uint32_t*)qkv,
+                          (uint32_t*)q_out, (uint32_t*)h->k_cache, (uint4*)h->v_cache, h->k_scale, h->v_scale, bt, qsl, ctx, R,
+                          c.max_pages_per_req, c.num_q_heads, c.num_kv_heads, c.head_dim, k, flag);
+    return launch_pdl(qkv_rope_append_kernel<false>, dim3((unsigned)T), dim3(kRopeThreads), 0, stream, (const uint32_t*)qkv,
+                      (uint32_t*)q_out, (uint32_t*)h->k_cache, (uint4*)h->v_cache, (const float*)nullptr, (const float*)nullptr, bt,
+                      qsl, ctx, R, c.max_pages_per_req, c.num_q_heads, c.num_kv_heads, c.head_dim, k, flag);
 }
 
 }  // namespace ss
