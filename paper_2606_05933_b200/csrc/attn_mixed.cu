@@ -3,7 +3,7 @@
 //
 // Persistent CTAs (one per SM) pull items from the device work list through a dynamic queue (atomic
 // counter), so tensor-bound prefill tiles and HBM-bound decode splits overlap across SMs and the batch
-// costs ~max(bytes/HBM, flops/tensor) instead of the sum.  12 warps per CTA in 3 warpgroups; the register
+// costs ~max(bytes/HBM, flops/tensor) instead of the sum.  12 warps per CTA in 3 warpgroups (bf16 cache); the register
 // file is re-partitioned with setmaxnreg (WG0 88 registers per thread, WG1 / WG2 208):
 //   WG0 warp 0  scheduler + Q / K producer (one elected thread).  Publishes each item to the other warps through a
 //               4-slot smem ring, loads the Q tiles (prefill: the item's 1 or 2 query heads, 128 rows each) and
@@ -32,9 +32,10 @@
 //                 cross-warp log-sum-exp merge through smem (G <= 8: one 8 -> 1 pass by all 256 threads; G > 8: WG2 ->
 //                 WG1 in registers, then 4 -> 1), then either the final bf16 row or an fp32 partial.
 //   FP8 cache (template FP8, SS_FLAG_KV_FP8): E4M3 codes through the same TMA boxes on 128-byte rows (6-slot rings).
-//               Decode: codes widened exactly to fp16 after ldmatrix, f16 mma.sync.  Prefill: single-head items; WG2's
-//               warps widen each staged tile into fp16 tiles in the bf16 slot layout for the tcgen05 MMAs (kind::f16 on
-//               fp16 operands), WG1 rewrites the Q tile as fp16 in place.
+//               Decode: codes widened exactly to fp16 after ldmatrix, f16 mma.sync; a warpgroup visits its own slots only.
+//               Prefill: a FOURTH warpgroup (16 warps; registers 88 / 192 / 192 / 40) widens each staged tile into fp16
+//               tiles in the bf16 slot layout for the tcgen05 MMAs (kind::f16 on fp16 operands) of both chains; each
+//               chain's workers rewrite their Q tile as fp16 in place.
 // Rooflines: decode items HBM (2*D*2 bytes per cached token per kv head), prefill items bf16 tensor
 // (4*D flop per visible (row,key) pair per head).  V rows at/after kv_end are zeroed in smem before any
 // PV product (unused slots may hold NaN; 0*NaN = NaN); masked scores are replaced, never multiplied.
@@ -58,17 +59,23 @@ namespace ss {
 
 using namespace ptx;
 
-constexpr int kMixThreads = 384;
 constexpr int kSlotKeys = 64;        // keys per K / V ring slot = keys per S buffer
 constexpr int kMaxSt = 8;            // most K / V ring slots of any instantiation (barrier index layout)
 constexpr int kBarBytes = 704;       // mbarrier block (8 bytes each)
 constexpr int kSchedSlots = 4;
 constexpr int kDecKeys = 16;         // keys of a 64-key slot one decode warp owns (4 warps per slot)
-// setmaxnreg moves registers inside the CTA's own launch allocation: 384 threads x 168 (the __launch_bounds__ cap ptxas
-// reports) = 64512, so 128*88 + 256*208 = 64512 fits exactly; one register more per worker and the .inc spins forever.
-// (88: the K producer thread keeps the next item, three tiles of page ids and its slot history without spilling.)
-constexpr int kRegsLaunch = 168, kRegsWg0 = 88, kRegsWorker = 208;
-static_assert(128 * kRegsWg0 + 256 * kRegsWorker <= kMixThreads * kRegsLaunch, "setmaxnreg.inc could never be granted");
+// setmaxnreg moves registers inside the CTA's own launch allocation.  bf16 cache: 384 threads x 168 (the __launch_bounds__
+// cap ptxas reports) = 64512, so 128*88 + 256*208 = 64512 fits exactly; one register more per worker and the .inc spins
+// forever.  (88: the K producer thread keeps the next item, three tiles of page ids and its slot history without spilling.)
+// FP8 cache: a fourth warpgroup (the fp8 -> fp16 tile converters of the prefill path) - 512 threads x 128 = 65536 =
+// 128*88 + 256*192 + 128*40.
+template <bool FP8>
+struct MixCta {
+    static constexpr int kThreads = FP8 ? 512 : 384;
+    static constexpr int kRegsLaunch = FP8 ? 128 : 168, kRegsWg0 = 88, kRegsWorker = FP8 ? 192 : 208, kRegsConv = 40;
+    static_assert(128 * kRegsWg0 + 256 * kRegsWorker + (FP8 ? 128 * kRegsConv : 0) <= kThreads * kRegsLaunch,
+                  "setmaxnreg.inc could never be granted");
+};
 constexpr float kMLog2e = 1.4426950408889634f;
 constexpr float kMLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.f;   // log2 units: P <= 2^8, safe in bf16 / fp32
@@ -139,7 +146,7 @@ enum : int {
     B_SCHED_FULL = B_PVDONE + 2, B_SCHED_EMPTY = B_SCHED_FULL + 4, B_PARTIAL = B_SCHED_EMPTY + 4,
     // FP8 prefill: fp16 copies of the staged tiles [buffer], and the Q tile converted in place
     B_KCONV_FULL = B_PARTIAL + 4, B_KCONV_EMPTY = B_KCONV_FULL + 2, B_VCONV_FULL = B_KCONV_EMPTY + 2,
-    B_VCONV_EMPTY = B_VCONV_FULL + 2, B_QCONV = B_VCONV_EMPTY + 2, B_COUNT = B_QCONV + 1
+    B_VCONV_EMPTY = B_VCONV_FULL + 2, B_QCONV = B_VCONV_EMPTY + 2 /* [chain] */, B_COUNT = B_QCONV + 2
 };
 static_assert(B_COUNT * 8 <= kBarBytes, "barrier region");
 static_assert(kSchedSlots == 4, "barrier indices assume 4 scheduler slots");
@@ -311,15 +318,34 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
     // always belongs to the same warpgroup: a warp waits and arrives on its own slots only, and sees every use of them.
     const int r16 = cw * kDecKeys;                          // first key row of this warp inside its slots
     const int mi = lane >> 3, l7 = lane & 7;                // ldmatrix: this lane addresses row l7 of matrix mi
+    // FP8: the swizzled ldmatrix offsets of this lane are loop invariants, pinned in registers (the empty asm makes them
+    // opaque: with the 128-register launch bound of the 16-warp CTA the compiler otherwise recomputes them per tile,
+    // +9 % instructions in a loop that is issue-bound)
+    uint32_t koffs[FP8 ? D / 32 : 1], voffs[FP8 ? D / 32 : 1];
+    if (FP8) {
+#pragma unroll
+        for (int jj = 0; jj < D / 32; ++jj) {
+            koffs[jj] = SM::kv_off(r16 + (mi & 1) * 8 + l7, 2 * jj + (mi >> 1));
+            voffs[jj] = SM::kv_off(r16 + (mi & 1) * 8 + l7, 2 * jj + (mi >> 1));
+            asm volatile("" : "+r"(koffs[jj]));
+            asm volatile("" : "+r"(voffs[jj]));
+        }
+    }
 #ifdef SS_PROFILE
     long long pf_t = clock64(), pf_acc[4] = {0, 0, 0, 0};     // K wait | S^T | V wait | softmax + O^T  (cycles, this warp)
 #endif
-    for (int t = 0; t < n; ++t) {
+    // even ring: only the item's tiles of this warpgroup's parity are visited, slot and phase parity advance by 2 slots
+    int s_run = (int)((tile_ctr + (uint32_t)wg) % SM::kNumSt);
+    uint32_t par_run = ((tile_ctr + (uint32_t)wg) / SM::kNumSt) & 1;
+    for (int t = SM::kOwnSlots ? wg : 0; t < n; t += SM::kOwnSlots ? 2 : 1) {
         const uint32_t tc = tile_ctr + t;
-        const int s = tc % SM::kNumSt;
-        const uint32_t fpar = (tc / SM::kNumSt) & 1;
+        const int s = SM::kOwnSlots ? s_run : (int)(tc % SM::kNumSt);
+        const uint32_t fpar = SM::kOwnSlots ? par_run : (tc / SM::kNumSt) & 1;
+        if (SM::kOwnSlots) {
+            s_run += 2;
+            if (s_run >= SM::kNumSt) { s_run -= SM::kNumSt; par_run ^= 1; }
+        }
         const int key0 = w.kv_begin + t * kSlotKeys;
-        if (SM::kOwnSlots && (t & 1) != wg) continue;          // even ring: the slot belongs to the other warpgroup
         // <= 0: nothing for this warp in this slot (odd ring: the other warpgroup's turn; it still waits and arrives)
         const int nvalid = (SM::kOwnSlots || (t & 1) == wg) ? w.kv_end - (key0 + r16) : 0;
         const uint32_t kbase = sbase + SM::kKOff + s * SM::kSlot;
@@ -342,7 +368,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
                 uint32_t r[D / 32][4];                           // one ldmatrix = 16 keys x 32 d of codes = two k-steps
 #pragma unroll
                 for (int jj = 0; jj < D / 32; ++jj)
-                    ldmatrix_x4(r[jj][0], r[jj][1], r[jj][2], r[jj][3], kbase + SM::kv_off(rk, 2 * jj + (mi >> 1)));
+                    ldmatrix_x4(r[jj][0], r[jj][1], r[jj][2], r[jj][3], kbase + koffs[jj]);
 #pragma unroll
                 for (int jj = 0; jj < D / 32; ++jj)
 #pragma unroll
@@ -393,7 +419,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
                 const int rv = r16 + (FP8 ? (mi & 1) : (mi >> 1)) * 8 + l7;
 #pragma unroll
                 for (int i = 0; i < kVLoads; ++i)
-                    ldmatrix_x4_trans(va[i][0], va[i][1], va[i][2], va[i][3], vbase + SM::kv_off(rv, 2 * i + (FP8 ? (mi >> 1) : (mi & 1))));
+                    ldmatrix_x4_trans(va[i][0], va[i][1], va[i][2], va[i][3], vbase + (FP8 ? voffs[FP8 ? i : 0] : SM::kv_off(rv, 2 * i + (mi & 1))));
             }
             uint32_t pb[NT][2];                              // B fragments of P^T (16 keys x 8 heads)
             bool moved = false;
@@ -727,7 +753,7 @@ __device__ __forceinline__ void split_merge(const ss_work_item& w, const int slo
 }
 
 template <int D, bool FP8>
-__global__ void __launch_bounds__(kMixThreads, 1)
+__global__ void __launch_bounds__(MixCta<FP8>::kThreads, 1)
 mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
              const __grid_constant__ CUtensorMap tmap_v, const MixParams prm) {
     using SM = MixSmem<D, FP8>;
@@ -750,7 +776,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         for (int s = 0; s < SM::kNumSt; ++s) {
             mbar_init(BAR(B_KFULL + s), 1);
             mbar_init(BAR(B_VFULL + s), 1);
-            mbar_init(BAR(B_KEMPTY_P + s), FP8 ? 1 : 2);     // one commit per chain; FP8: the K converter pair
+            mbar_init(BAR(B_KEMPTY_P + s), FP8 ? 1 : 2);     // one commit per chain; FP8: the K converter warps
             mbar_init(BAR(B_VEMPTY_P + s), FP8 ? 1 : 2);
             mbar_init(BAR(B_KEMPTY_D + s), SM::kOwnSlots ? 4 : 8);   // the owning warpgroup / every decode warp
             mbar_init(BAR(B_VEMPTY_D + s), SM::kOwnSlots ? 4 : 8);
@@ -764,11 +790,12 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         if (FP8) {
             for (int b = 0; b < 2; ++b) {
                 mbar_init(BAR(B_KCONV_FULL + b), 1);
-                mbar_init(BAR(B_KCONV_EMPTY + b), 1);
+                mbar_init(BAR(B_KCONV_EMPTY + b), 2);             // one commit per chain, like the ring slots
                 mbar_init(BAR(B_VCONV_FULL + b), 1);
-                mbar_init(BAR(B_VCONV_EMPTY + b), 1);
+                mbar_init(BAR(B_VCONV_EMPTY + b), 2);
             }
-            mbar_init(BAR(B_QCONV), 128);
+            mbar_init(BAR(B_QCONV + 0), 128);
+            mbar_init(BAR(B_QCONV + 1), 128);
         }
         for (int x = 0; x < 2; ++x) {
             mbar_init(BAR(B_OFULL + x), 1);
@@ -778,7 +805,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         for (int s = 0; s < kSchedSlots; ++s) {
             mbar_init(BAR(B_PARTIAL + s), G <= 8 ? 256 : 128);   // the threads that store decode partials (see decode_item)
             mbar_init(BAR(B_SCHED_FULL + s), 1);
-            mbar_init(BAR(B_SCHED_EMPTY + s), 11);               // 2 MMA warps (warp 2 = a5) + the V producer + 8 worker warps
+            mbar_init(BAR(B_SCHED_EMPTY + s), FP8 ? 15 : 11);    // 2 MMA warps (warp 2 = a5) + the V producer + 8 worker warps (+ 4 converter warps)
         }
         fence_barrier_init();
         prefetch_tmap(&tmap_q);
@@ -803,8 +830,8 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         if (threadIdx.x == 0) { ph->tot_p = 0; ph->tot_d = 0; ph->n_decode_ctas = 0; ph->nP = 0; ph->nD = 0; }
     } else if (prm.self_plan) {
         // a2: every CTA builds the same plan (scratch = the still unused K ring); items are decoded from queue tickets
-        build_plan<kMixThreads, uint16_t>(prm.qsl, prm.ctx_lens, prm.R, Hq, Hkv, D, prm.num_sms, prm.force_split_keys,
-                                          prm.force_decode_ctas, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph, FP8 ? 1 : 0);   // FP8: single-head prefill items
+        build_plan<MixCta<FP8>::kThreads, uint16_t>(prm.qsl, prm.ctx_lens, prm.R, Hq, Hkv, D, prm.num_sms, prm.force_split_keys,
+                                          prm.force_decode_ctas, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph);
         fence_proxy_async();    // scratch was written through the generic proxy; TMA writes the same bytes next
     } else if (threadIdx.x == 0) {
         ph->tot_p = prm.hdr->n_prefill;
@@ -819,7 +846,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     // setmaxnreg sit INSIDE the role branches (which only re-join at the teardown): ptxas allocates each region against
     // the count of the setmaxnreg that dominates it, and code reachable from both would get the smaller one.
     if (warp < 4) {
-      setmaxnreg_dec<kRegsWg0>();
+      setmaxnreg_dec<MixCta<FP8>::kRegsWg0>();
       if (warp == 0) {
         // =============================== scheduler + TMA producer ===============================
         // One elected thread runs the whole loop (waits included) so every TMA operand is uniform.
@@ -955,8 +982,9 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         // for both chains.  The chains touch disjoint TMEM and only read the shared K/V slots, so no order is needed
         // between them; the slot / Q-tile release barriers take one commit per chain (chain A commits twice when the
         // item has a single head).  Decode items: warp 1 has nothing to do, warp 2 runs a5 (split_merge).
-        // FP8 cache: prefill items have one head (chain A); the operands are the fp16 copies the converter warps (WG2) write
-        // into two K and two V buffers, Q converted in place by chain A's workers; tiles are counted by cv_ctr.
+        // FP8 cache: the operands are the fp16 copies the converter warps (WG3) write into two K and two V buffers (shared
+        // by both chains, released by one commit per chain), Q converted in place by each chain's workers; tiles are
+        // counted by cv_ctr.
         constexpr uint32_t idesc_qk = FP8 ? umma_idesc_f16(kTileRows, kSlotKeys, 0) : umma_idesc_bf16(kTileRows, kSlotKeys, 0);
         constexpr uint32_t idesc_pv = FP8 ? umma_idesc_f16(kTileRows, D, 1) : umma_idesc_bf16(kTileRows, D, 1);
         const int X = warp - 1;
@@ -978,6 +1006,10 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             if (kind == 0) break;
             if (kind == 1) {
                 const int nq = w.nheads;
+                // Every issuer observes every Q phase, also chain B's on a single-head item it sits out: a parity wait
+                // is only exact for a waiter that is at most one phase behind, and the Q phase is what orders an item
+                // against the ring (see B_QEMPTY below).
+                if (X >= nq && elect_one()) mbar_wait(BAR(B_QFULL), n_pre & 1);
                 if (X < nq && elect_one()) {
                     const int ncommit = nq == 1 ? 2 : 1;          // arrivals this chain owes the shared (count 2) barriers
 #ifdef SS_PROFILE
@@ -1003,7 +1035,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                             umma_ss(tchain + b * 64, qdesc0 + (qoff >> 4), kdesc0 + (koff >> 4), idesc_qk, ks > 0);
                         }
                         umma_commit(BAR(B_SFULL + X * 2 + b));
-                        if (FP8) umma_commit(BAR(B_KCONV_EMPTY + cb));
+                        if (FP8) for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_KCONV_EMPTY + cb));
                         else for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_KEMPTY_P + s));
                     };
                     auto issue_pv = [&](int kt) {
@@ -1026,7 +1058,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         for (int kk = 0; kk < kSlotKeys / 16; ++kk)      // A = P[b] from TMEM: 16 keys = 8 packed columns
                             umma_ts(tchain + SM::kTmemO, tchain + b * 64 + kk * 8, vdesc0 + (uint64_t)(kk * kstep >> 4), idesc_pv, (kt > 0 || kk > 0));
                         umma_commit(BAR(B_PVDONE + X));
-                        if (FP8) umma_commit(BAR(B_VCONV_EMPTY + cb));
+                        if (FP8) for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_VCONV_EMPTY + cb));
                         else for (int c = 0; c < ncommit; ++c) umma_commit(BAR(B_VEMPTY_P + s));
                         if (kt == nr - 1) {
                             umma_commit(BAR(B_OFULL + X));
@@ -1038,7 +1070,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         }
                     };
                     mbar_wait(BAR(B_QFULL), n_pre & 1);
-                    if (FP8) { mbar_wait(BAR(B_QCONV), n_pre & 1); tc_fence_after(); }       // Q tile rewritten as fp16
+                    if (FP8) { mbar_wait(BAR(B_QCONV + X), n_chain & 1); tc_fence_after(); }   // this chain's Q tile rewritten as fp16
 #ifdef SS_PROFILE
                     mm_t = clock64();
 #endif
@@ -1068,8 +1100,8 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         }
         if (trace && lane == 0 && X == 1) trace[4] = globaltimer_ns();
       }
-    } else {
-        setmaxnreg_inc<kRegsWorker>();
+    } else if (warp < 12) {
+        setmaxnreg_inc<MixCta<FP8>::kRegsWorker>();
         // =============================== workers ===============================
         const int wg = (warp - 4) >> 2;                        // 0: chain A / decode on even slots, 1: chain B / decode on odd slots
         const int cw = (warp - 4) & 3;                         // decode: 16-key slice of the slot
@@ -1080,8 +1112,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
         const float sl2_base = prm.scale * kMLog2e;
         const uint32_t tchain = tmem_base + wg * SM::kTmemChain;
         const uint32_t tmem_o = tchain + SM::kTmemO;
-        uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_chain = 0;
-        uint32_t cv_ctr = 0;                                   // FP8 converters (WG2): prefill tiles converted so far
+        uint32_t tile_ctr = 0, s_ctr = 0, n_sched = 0, n_chain = 0, n_pre = 0;
         float* merge = reinterpret_cast<float*>(smem + SM::kQOff);
         if (wg == 0 && G > 8) named_bar_arrive(3, 256);        // G > 8: the decode merge buffer starts out free (stage A of decode_item)
         for (;;) {
@@ -1101,12 +1132,15 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 tr[2] = ((unsigned long long)w.kind << 32) | (unsigned)n;
             }
             const int nr = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;      // real tiles (n may hold a padding tile)
+            if (FP8 && w.kind == 1) {
+                mbar_wait(BAR(B_QFULL), n_pre & 1);        // every Q phase, also by a chain that sits the item out (exact parity)
+                ++n_pre;
+            }
             if (w.kind == 1 && wg < w.nheads) {
                 // -------------------------- prefill tile, chain wg: thread = query row --------------------------
                 if (FP8) {
                     // FP8 cache: the MMAs run on fp16 operands - this chain's Q tile is rewritten in place (same swizzled
                     // positions, bf16 -> fp16: exact for magnitudes in [2^-14, 65504], clamped above) before the first S
-                    mbar_wait(BAR(B_QFULL), n_chain & 1);
                     uint8_t* qt = smem + SM::kQOff + wg * SM::kQTile;
                     for (int i = wtid; i < SM::kQTile / 16; i += 128) {
                         uint4 v = *reinterpret_cast<uint4*>(qt + i * 16);
@@ -1114,7 +1148,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                         *reinterpret_cast<uint4*>(qt + i * 16) = v;
                     }
                     fence_proxy_async();
-                    mbar_arrive(BAR(B_QCONV));
+                    mbar_arrive(BAR(B_QCONV + wg));
                 }
                 const float sl2 = sl2_base * (FP8 ? __ldg(prm.k_scale + w.head / G) : 1.f);
                 const int u = __ldg(prm.ctx_lens + w.req);
@@ -1223,48 +1257,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
                 s_ctr += nr;
                 ++n_chain;
             } else if (w.kind == 1) {
-                // single-head item: chain B has nothing to do - except over an FP8 cache, where its four warps widen the
-                // staged tiles to fp16 for the tensor cores: warps 0, 1 the K tiles, warps 2, 3 the V tiles, each pair at
-                // its own pace (K(t) needs S(t-2) done, V(t) needs PV(t-2) done).  A 16-byte chunk of codes becomes two
-                // chunks of the fp16 tile (same swizzled slot layout as a bf16 tile); rows past kv_end are written as
-                // zeros (unused slots may hold NaN codes; 0 * NaN = NaN in the PV product).
-                if (FP8) {
-                    const int is_v = cw >> 1;
-                    const int ct = (cw & 1) * 32 + lane;                                  // 0 .. 63 inside the pair
-                    const uint32_t ring = sbase + (is_v ? SM::kVOff : SM::kKOff);
-                    const uint32_t conv = sbase + (is_v ? SM::kVConvOff : SM::kKConvOff);
-                    const int b_full = is_v ? B_VFULL : B_KFULL, b_empty = is_v ? B_VEMPTY_P : B_KEMPTY_P;
-                    const int c_full = is_v ? B_VCONV_FULL : B_KCONV_FULL, c_empty = is_v ? B_VCONV_EMPTY : B_KCONV_EMPTY;
-                    for (int t = 0; t < n; ++t) {                                         // ring tiles, padding tile included
-                        const uint32_t tc = tile_ctr + t;
-                        const int s = tc % SM::kNumSt;
-                        mbar_wait(BAR(b_full + s), (tc / SM::kNumSt) & 1);
-                        const uint32_t cv = cv_ctr + t, cb = cv & 1;
-                        if (t < nr) {
-                            mbar_wait(BAR(c_empty + cb), ((cv >> 1) & 1) ^ 1);            // the MMAs that read this buffer are done
-                            const int nkeys = w.kv_end - t * kSlotKeys;
-                            const uint32_t src = ring + s * SM::kSlot, dst = conv + cb * SM::kConvTile;
-#pragma unroll 4
-                            for (int q = ct; q < kSlotKeys * 8; q += 64) {
-                                const int r = q >> 3, cd = q & 7;
-                                uint32_t c0 = 0u, c1 = 0u, c2 = 0u, c3 = 0u;
-                                if (r < nkeys)
-                                    asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(c0), "=r"(c1), "=r"(c2), "=r"(c3) : "r"(src + SM::kv_off(r, cd)));
-                                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + SM::conv_off(r, 2 * cd)), "r"(e4m3x2_to_f16x2(c0)),
-                                             "r"(e4m3x2_hi_to_f16x2(c0)), "r"(e4m3x2_to_f16x2(c1)), "r"(e4m3x2_hi_to_f16x2(c1)) : "memory");
-                                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + SM::conv_off(r, 2 * cd + 1)), "r"(e4m3x2_to_f16x2(c2)),
-                                             "r"(e4m3x2_hi_to_f16x2(c2)), "r"(e4m3x2_to_f16x2(c3)), "r"(e4m3x2_hi_to_f16x2(c3)) : "memory");
-                            }
-                            fence_proxy_async();                                          // generic writes -> the MMA's async proxy
-                        }
-                        named_bar_sync(4 + is_v, 64);
-                        if (ct == 0) {
-                            if (t < nr) mbar_arrive(BAR(c_full + cb));
-                            mbar_arrive(BAR(b_empty + s));                                // the ring slot is free
-                        }
-                    }
-                    cv_ctr += nr;
-                }
+                // single-head item: chain B has nothing to do
             } else {
                 // -------------------------- decode split: all 8 worker warps --------------------------
                 // Warp dw owns 16 keys of every other 64-key slot: warps 0-3 (WG1) the even slots of the item, warps 4-7
@@ -1284,6 +1277,69 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
             if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
         }
         if (trace && wg == 0 && wtid == 0) { trace[2] = globaltimer_ns(); trace[3] = n_sched - 1; }
+    } else if constexpr (FP8) {
+        // =============================== fp8 -> fp16 tile converters (FP8 cache only) ===============================
+        // The tcgen05 MMAs of a prefill item run on fp16 operands: warps 12, 13 widen every staged K tile, warps 14, 15
+        // every V tile, into two K and two V buffers in the bf16 slot layout, each pair at its own pace (K(t) needs
+        // S(t-2) of both chains done, V(t) needs PV(t-2)).  A 16-byte chunk of codes becomes two chunks of the fp16
+        // tile; rows past kv_end are written as zeros (unused slots may hold NaN codes; 0 * NaN = NaN in the PV
+        // product).  Decode items are sat out (their warps widen in registers), so every prefill item starts with its
+        // Q phase: once that Q tile has landed, every ring tile issued before it has landed and been released, and the
+        // parity waits on the ring are exact again.
+        setmaxnreg_dec<MixCta<FP8>::kRegsConv>();
+        const int cw = warp - 12;
+        const int is_v = cw >> 1;
+        const int ct = (cw & 1) * 32 + lane;                                  // 0 .. 63 inside the pair
+        const uint32_t ring = sbase + (is_v ? SM::kVOff : SM::kKOff);
+        const uint32_t conv = sbase + (is_v ? SM::kVConvOff : SM::kKConvOff);
+        const int b_full = is_v ? B_VFULL : B_KFULL, b_empty = is_v ? B_VEMPTY_P : B_KEMPTY_P;
+        const int c_full = is_v ? B_VCONV_FULL : B_KCONV_FULL, c_empty = is_v ? B_VCONV_EMPTY : B_KCONV_EMPTY;
+        uint32_t tile_ctr = 0, n_sched = 0, cv_ctr = 0, n_pre = 0;
+        for (;;) {
+            const int slot = n_sched % kSchedSlots;
+            mbar_wait(BAR(B_SCHED_FULL + slot), (n_sched / kSchedSlots) & 1);
+            const ss_work_item w = sched[slot];
+            ++n_sched;
+            if (w.kind == 0) break;
+            const int nr = (w.kv_end - w.kv_begin + kSlotKeys - 1) / kSlotKeys;      // real tiles
+            const int n = (nr + 1) & ~1;                                             // ring tiles (even ring: padded)
+            if (w.kind == 1) {
+                mbar_wait(BAR(B_QFULL), n_pre & 1);
+                ++n_pre;
+                for (int t = 0; t < n; ++t) {
+                    const uint32_t tc = tile_ctr + t;
+                    const int s = tc % SM::kNumSt;
+                    mbar_wait(BAR(b_full + s), (tc / SM::kNumSt) & 1);
+                    const uint32_t cv = cv_ctr + t, cb = cv & 1;
+                    if (t < nr) {
+                        mbar_wait(BAR(c_empty + cb), ((cv >> 1) & 1) ^ 1);            // the MMAs that read this buffer are done
+                        const int nkeys = w.kv_end - t * kSlotKeys;
+                        const uint32_t src = ring + s * SM::kSlot, dst = conv + cb * SM::kConvTile;
+#pragma unroll 4
+                        for (int q = ct; q < kSlotKeys * 8; q += 64) {
+                            const int r = q >> 3, cd = q & 7;
+                            uint32_t c0 = 0u, c1 = 0u, c2 = 0u, c3 = 0u;
+                            if (r < nkeys)
+                                asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(c0), "=r"(c1), "=r"(c2), "=r"(c3) : "r"(src + SM::kv_off(r, cd)));
+                            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + SM::conv_off(r, 2 * cd)), "r"(e4m3x2_to_f16x2(c0)),
+                                         "r"(e4m3x2_hi_to_f16x2(c0)), "r"(e4m3x2_to_f16x2(c1)), "r"(e4m3x2_hi_to_f16x2(c1)) : "memory");
+                            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(dst + SM::conv_off(r, 2 * cd + 1)), "r"(e4m3x2_to_f16x2(c2)),
+                                         "r"(e4m3x2_hi_to_f16x2(c2)), "r"(e4m3x2_to_f16x2(c3)), "r"(e4m3x2_hi_to_f16x2(c3)) : "memory");
+                        }
+                        fence_proxy_async();                                          // generic writes -> the MMA's async proxy
+                    }
+                    named_bar_sync(4 + is_v, 64);
+                    if (ct == 0) {
+                        if (t < nr) mbar_arrive(BAR(c_full + cb));
+                        mbar_arrive(BAR(b_empty + s));                                // the ring slot is free
+                    }
+                }
+                cv_ctr += nr;
+            }
+            tile_ctr += n;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(BAR(B_SCHED_EMPTY + slot));
+        }
     }
 
     // ---- teardown ----
@@ -1366,11 +1422,11 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     const int grid = h->dbg[kDbgGrid] > 0 ? h->dbg[kDbgGrid] : h->num_sms;
     cudaError_t e;
     if (h->kv_fp8)
-        e = launch_pdl(mixed_kernel<128, true>, dim3(grid), dim3(kMixThreads), MixSmem<128, true>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+        e = launch_pdl(mixed_kernel<128, true>, dim3(grid), dim3(MixCta<true>::kThreads), MixSmem<128, true>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
     else if (c.head_dim == 128)
-        e = launch_pdl(mixed_kernel<128, false>, dim3(grid), dim3(kMixThreads), MixSmem<128>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+        e = launch_pdl(mixed_kernel<128, false>, dim3(grid), dim3(MixCta<false>::kThreads), MixSmem<128>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
     else
-        e = launch_pdl(mixed_kernel<64, false>, dim3(grid), dim3(kMixThreads), MixSmem<64>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
+        e = launch_pdl(mixed_kernel<64, false>, dim3(grid), dim3(MixCta<false>::kThreads), MixSmem<64>::kTotal, stream, tmap_q, h->tmap_k, h->tmap_v, p);
     if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }

@@ -54,7 +54,7 @@ __device__ __forceinline__ int plan_decode_chunk(int n, int L) {
 template <int NT, typename OffT>
 __device__ void build_plan(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int Hq, int Hkv,
                            int D, int num_sms, int force_split_keys, int force_decode_ctas, int32_t* scratch,
-                           PlanTables<OffT> tb, PlanHeader* ph, int no_pairs = 0) {
+                           PlanTables<OffT> tb, PlanHeader* ph) {
     int32_t* s_c = scratch;
     int32_t* s_u = scratch + R;
     int32_t* s_cost = scratch + 2 * ((R + 3) & ~3);          // 16-byte aligned: read as int4
@@ -173,8 +173,7 @@ __device__ void build_plan(const int32_t* __restrict__ qsl, const int32_t* __res
             }
             if (force_decode_ctas > 0) nd = force_decode_ctas;
             if (force_decode_ctas < 0) nd = 0;
-            // no_pairs: FP8 cache - chain B's warps convert the staged tiles to fp16, so an item serves one head
-            const int pair = no_pairs ? 0 : plan_pair_heads(tiles_p, Hq, Hkv, num_sms - (nd < num_sms ? nd : 0));
+            const int pair = plan_pair_heads(tiles_p, Hq, Hkv, num_sms - (nd < num_sms ? nd : 0));
             ph->pair_heads = pair;
             const int tot_p = tiles_p * (pair ? plan_head_pairs(Hq, Hkv) : Hq);
             ph->tot_p = tot_p;

@@ -265,12 +265,41 @@ def _edge_rows(b, per_req=24, seed=0):
     ([(65, 4031), (64, 64), (1, 4095)], (28, 4, 128)),        # G = 7: odd group, single-head items
     ([(2048, 4096)], (32, 8, 128)),                           # PP-b
     ([(1024, 0), (1024, 6000), (1, 3000), (1, 9000)], (64, 8, 128)),   # 70B shape, PP-f + decodes
+    ([(700, 300), (300, 0), (1, 2000), (1, 17)], (28, 4, 128)),        # G = 7 with head pairs: 3 pair items + 1 single-head item per kv head
+    ([(640, 0), (1, 100)], (6, 2, 128)),                               # G = 3, too few items to pair: single-head items only
 ])
 def test_fp8_prefill_on_tensor_cores(reqs, shape):
-    """Prefill chunks over the FP8 cache: tcgen05 on fp16 copies of the staged tiles (converter warps), single-head items."""
+    """Prefill chunks over the FP8 cache: tcgen05 on fp16 copies of the staged tiles (converter warpgroup); single-head items
+    while one wave of CTAs holds them all, head pairs (two chains on one converted tile) from the second wave on."""
     Hq, Hkv, D = shape
     b = wl.make_batch("fp8-prefill", Hq, Hkv, D, reqs, 90 + len(reqs), with_append=True)
     fp8_case(b, seed=len(reqs), check_rows=_edge_rows(b) if b.T > 700 else None)
+
+
+@pytest.mark.parametrize("fp8", [False, True])
+def test_single_head_item_as_long_as_the_ring_then_a_pair_item(fp8):
+    """G = 7, forty 128-row chunks whose items cover exactly as many ring tiles as the ring has slots (5 over the bf16 cache;
+    5 + the padding tile = 6 over the FP8 cache): chain B sits out every fourth item and then takes a pair item whose
+    first tile reuses the slot of the skipped item's first tile - its issuer must have seen every Q phase for the parity
+    waits on the ring to be exact (a race the build before the fix did not lose on this batch either: the test pins the
+    shape, the argument is in attn_mixed.cu).  Five launches, all rows against the oracle."""
+    rng = np.random.default_rng(4242)
+    reqs = [(128, int(u)) for u in rng.integers(130, 192, size=40, endpoint=True)] + [(1, 300), (1, 5000)]
+    b = wl.make_batch("single-then-pair", 28, 4, 128, reqs, 4242, with_append=True)
+    if fp8:
+        fp8_case(b, seed=42)
+        return
+    t = wl.make_tensors(b, DEV, poison_unused=True)
+    k0, v0 = wl.to_u16(t.k_cache), wl.to_u16(t.v_cache)
+    h = binding.handle_for(b, t)
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    binding.kv_append(h, t.k_new, t.v_new, bt, qsl, ctx)
+    outs = [binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale).clone() for _ in range(5)]
+    torch.cuda.synchronize()
+    oracle.kv_append(k0, v0, wl.to_u16(t.k_new), wl.to_u16(t.v_new), b.block_table, b.query_start_loc, b.ctx_lens)
+    ref, _, _ = oracle.mixed_attention(wl.to_u16(t.q), k0, v0, b.block_table, b.query_start_loc, b.ctx_lens, b.scale)
+    for out in outs:
+        check_attention(b, out, ref)
 
 
 def test_randomized_shapes_and_mixes_bf16_and_fp8():
