@@ -88,6 +88,10 @@ def surface_points(with_c4: bool = False, dense: bool = False, model: Optional[s
     pts.append(("C2", wl.config_c2))
     pts.append(("C2-shuffled", lambda: wl.config_c2(shuffle=True)))
     pts.append(("C5", wl.config_c5))
+    for name in ("PP-b", "PP-e", "PP-f"):                  # prefill and mixed batches over the FP8 cache
+        pts.append((name + "/fp8", lambda name=name: fp8_variant(wl.config_scene_edge(name))))
+    pts.append(("C2/fp8", lambda: fp8_variant(wl.config_c2())))
+    pts.append(("C5/fp8", lambda: fp8_variant(wl.config_c5())))
     if with_c4:
         pts.append(("C4", wl.config_c4))
         pts.append(("C4/fp8", lambda: fp8_variant(wl.config_c4())))
