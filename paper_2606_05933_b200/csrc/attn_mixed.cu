@@ -318,18 +318,17 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
     // always belongs to the same warpgroup: a warp waits and arrives on its own slots only, and sees every use of them.
     const int r16 = cw * kDecKeys;                          // first key row of this warp inside its slots
     const int mi = lane >> 3, l7 = lane & 7;                // ldmatrix: this lane addresses row l7 of matrix mi
-    // FP8: the swizzled ldmatrix offsets of this lane are loop invariants, pinned in registers (the empty asm makes them
-    // opaque: with the 128-register launch bound of the 16-warp CTA the compiler otherwise recomputes them per tile,
-    // +9 % instructions in a loop that is issue-bound)
-    uint32_t koffs[FP8 ? D / 32 : 1], voffs[FP8 ? D / 32 : 1];
-    if (FP8) {
+    // The swizzled ldmatrix offsets of this lane are loop invariants, pinned in registers (the empty asm makes them opaque:
+    // the compiler otherwise recomputes them per tile - FP8 under the 128-register launch bound of the 16-warp CTA: +9 %
+    // instructions in a loop that is issue-bound; bf16: ~90 of the loop's 376 instructions)
+    constexpr int kFragLoads = FP8 ? D / 32 : D / 16;           // ldmatrix.x4 per tensor per 16-key slice
+    uint32_t koffs[kFragLoads], voffs[kFragLoads];
 #pragma unroll
-        for (int jj = 0; jj < D / 32; ++jj) {
-            koffs[jj] = SM::kv_off(r16 + (mi & 1) * 8 + l7, 2 * jj + (mi >> 1));
-            voffs[jj] = SM::kv_off(r16 + (mi & 1) * 8 + l7, 2 * jj + (mi >> 1));
-            asm volatile("" : "+r"(koffs[jj]));
-            asm volatile("" : "+r"(voffs[jj]));
-        }
+    for (int jj = 0; jj < kFragLoads; ++jj) {
+        koffs[jj] = SM::kv_off(r16 + (mi & 1) * 8 + l7, 2 * jj + (mi >> 1));
+        voffs[jj] = FP8 ? SM::kv_off(r16 + (mi & 1) * 8 + l7, 2 * jj + (mi >> 1)) : SM::kv_off(r16 + (mi >> 1) * 8 + l7, 2 * jj + (mi & 1));
+        asm volatile("" : "+r"(koffs[jj]));
+        asm volatile("" : "+r"(voffs[jj]));
     }
 #ifdef SS_PROFILE
     long long pf_t = clock64(), pf_acc[4] = {0, 0, 0, 0};     // K wait | S^T | V wait | softmax + O^T  (cycles, this warp)
@@ -361,7 +360,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
             for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
                 for (int i = 0; i < 4; ++i) sT[nt][i] = sU[nt][i] = 0.f;
-            const int rk = r16 + (mi & 1) * 8 + l7;          // a0: keys 0-7, a1: keys 8-15, a2 / a3: the next 8 d
+            // lane's K row: r16 + (mi & 1) * 8 + l7 - a0: keys 0-7, a1: keys 8-15, a2 / a3: the next 8 d (offsets in koffs)
             // every fragment load is issued before the first MMA (the wrappers are asm volatile and keep their order: an
             // interleaved loop exposed one ldmatrix latency per k-step)
             if (FP8) {
@@ -383,7 +382,7 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
                 uint32_t a[D / 16][4];
 #pragma unroll
                 for (int ks = 0; ks < D / 16; ++ks)
-                    ldmatrix_x4(a[ks][0], a[ks][1], a[ks][2], a[ks][3], kbase + SM::kv_off(rk, 2 * ks + (mi >> 1)));
+                    ldmatrix_x4(a[ks][0], a[ks][1], a[ks][2], a[ks][3], kbase + koffs[ks]);
 #pragma unroll
                 for (int ks = 0; ks < D / 16; ++ks)
 #pragma unroll
@@ -415,12 +414,9 @@ __device__ __forceinline__ void decode_item(const ss_work_item& w, const int n, 
             // FP8: matrices (keys 0-7, chunk), (keys 8-15, chunk), the same for chunk + 1, one ldmatrix per 32 d
             constexpr int kVLoads = FP8 ? D / 32 : D / 16;
             uint32_t va[kVLoads][4];
-            {
-                const int rv = r16 + (FP8 ? (mi & 1) : (mi >> 1)) * 8 + l7;
 #pragma unroll
-                for (int i = 0; i < kVLoads; ++i)
-                    ldmatrix_x4_trans(va[i][0], va[i][1], va[i][2], va[i][3], vbase + (FP8 ? voffs[FP8 ? i : 0] : SM::kv_off(rv, 2 * i + (mi & 1))));
-            }
+            for (int i = 0; i < kVLoads; ++i)
+                ldmatrix_x4_trans(va[i][0], va[i][1], va[i][2], va[i][3], vbase + voffs[i]);
             uint32_t pb[NT][2];                              // B fragments of P^T (16 keys x 8 heads)
             bool moved = false;
             float mn[NT][2];
