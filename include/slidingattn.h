@@ -151,6 +151,42 @@ int ss_mixed_attention(ss_handle* h, const void* q, const int32_t* block_table,
                        size_t workspace_bytes, void* cuda_stream);
 
 /*
+ * ss_mixed_attention for callers that CANNOT ALLOCATE device memory.  Who that is: a serving engine that gives every
+ * free byte of HBM to its paged KV cache when it starts has nothing left for a cudaMalloc by the time an iteration
+ * runs; a plugin living inside someone else's memory pool may not be allowed one; and a cudaMalloc on the iteration
+ * path stalls the whole device.  The regular route allocates twice on such a caller's behalf (ss_create mallocs the
+ * handle's counters, and somebody has to malloc the workspace).  This entry point needs neither: no handle, no
+ * workspace, and it calls no cudaMalloc / cudaFree or any other allocating routine.  Its scratch is an array compiled
+ * into the library: SS_STATIC_SCRATCH_BYTES of device memory on every GPU that loads the library, held until the
+ * process exits whether or not this function is ever called.
+ *
+ * Same operation, same kernels, same results as ss_mixed_attention (a2..a5 above) on a handle created with this `cfg`,
+ * flags == 0 and these caches; the caches must already hold the batch's u_r + c_r tokens.  Inputs and outputs are still
+ * the caller's device memory.
+ *   cfg                flags must be 0 (bf16 cache, no device checks).  The scratch a config needs grows with
+ *                      max_requests, max_tokens, max_pages_per_req and the head counts exactly as ss_workspace_bytes
+ *                      does (plus 4 * (8 + max_requests * num_kv_heads) bytes of counters).  A config that needs more than
+ *                      SS_STATIC_SCRATCH_BYTES is refused with SS_ERR_WORKSPACE_TOO_SMALL and both byte counts in
+ *                      err_msg; nothing is launched.  Guide: Llama-3-8B shapes (32 / 8 heads, D = 128) with 129 requests,
+ *                      2176 tokens and 8K context need 5.1 MB; the 70B batch C5 (64 / 8 heads, 30K context) needs 21 MB
+ *                      and does not fit - so size cfg to the iteration's real bounds, not the engine's global ones.
+ *   err_msg            optional host buffer (err_msg_len bytes) that receives a one-line reason on any non-zero return.
+ * FIRST CALL ON EACH DEVICE does a one-time set-up with that device current (looks up the array's device address,
+ * reads the SM count, sets the kernels' shared-memory attribute).  Make that first call during start-up, outside any
+ * stream capture; it needs real arguments, so a small warm-up batch is the way to do it.
+ * SHARED STATE: every call on a device uses the same array, and the array keeps the previous call's contents.  The
+ * call itself clears (cudaMemsetAsync on `cuda_stream`) the counters that must start at zero; everything else is
+ * written before it is read.  Two calls whose GPU work overlaps - different streams, or different host threads on one
+ * device - race on the array and produce garbage: order them on one stream or by events.  Calls on ss_create handles
+ * do not touch the array and may overlap with it freely.
+ */
+#define SS_STATIC_SCRATCH_BYTES (8u << 20)
+int ss_mixed_attention_static(const ss_config* cfg, void* k_cache_device, void* v_cache_device, const void* q,
+                              const int32_t* block_table, const int32_t* query_start_loc, const int32_t* ctx_lens,
+                              int32_t R, int32_t T, float scale, void* out, float* lse_or_null, void* cuda_stream,
+                              char* err_msg, size_t err_msg_len);
+
+/*
  * End-to-end iteration from HOST buffers (what a serving loop without device-resident activations
  * calls; bench.py's "e2e" leg): copies q / k_new / v_new / metadata host->device into handle-owned
  * staging buffers, runs ss_kv_append (if k_new_host != NULL) and ss_mixed_attention, copies `out`

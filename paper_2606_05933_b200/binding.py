@@ -22,7 +22,7 @@ SS_FLAG_KV_FP8 = 2
 # include/slidingattn.h (the product boundary) ...
 EXPORTS = ["ss_version", "ss_status_string", "ss_last_error_string", "ss_create", "ss_destroy",
            "ss_workspace_bytes", "ss_set_kv_scales", "ss_kv_append", "ss_qkv_rope_append", "ss_mixed_attention",
-           "ss_iteration_host",
+           "ss_mixed_attention_static", "ss_iteration_host",
            "ss_poll_device_error", "ss_reset"]
 # ... and include/slidingattn_debug.h (test / tuning / measurement aids)
 DEBUG_EXPORTS = ["ss_build_worklist", "ss_last_launch_count", "ss_debug_force_simple_path",
@@ -73,6 +73,8 @@ def load():
     lib.ss_kv_append.argtypes = [vp, vp, vp, vp, vp, vp, i32, i32, vp]
     lib.ss_qkv_rope_append.argtypes = [vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
     lib.ss_mixed_attention.argtypes = [vp, vp, vp, vp, vp, i32, i32, f32, vp, vp, vp, ctypes.c_size_t, vp]
+    lib.ss_mixed_attention_static.argtypes = [ctypes.POINTER(ss_config), vp, vp, vp, vp, vp, vp, i32, i32, f32, vp, vp,
+                                              vp, ctypes.c_char_p, ctypes.c_size_t]
     lib.ss_build_worklist.argtypes = [vp, vp, vp, i32, i32, vp, ctypes.c_size_t, vp, i32,
                                       ctypes.POINTER(i32 * 3), vp]
     lib.ss_iteration_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, i32, f32, vp, vp]
@@ -287,6 +289,45 @@ def mixed_attention(handle: SlidingAttn, q, block_table, query_start_loc, ctx_le
     """north_star mixed_attention(q, k_cache, v_cache, block_table, query_start_loc, ctx_lens, scale, out);
     the caches are the ones the handle was created on."""
     return handle.mixed_attention(q, block_table, query_start_loc, ctx_lens, scale, out, lse, stream)
+
+
+STATIC_SCRATCH_BYTES = 8 << 20      # SS_STATIC_SCRATCH_BYTES
+
+
+def mixed_attention_static(k_cache, v_cache, q, block_table, query_start_loc, ctx_lens, scale, max_requests=None,
+                           max_tokens=None, out=None, lse=None, stream=None):
+    """ss_mixed_attention_static: mixed_attention with no handle and no workspace, for callers that cannot allocate
+    device memory (an engine whose KV cache already owns all of HBM, code inside another framework's pool).  The
+    scratch is a STATIC_SCRATCH_BYTES array inside the library, shared by every call on the device: calls must not
+    overlap on the GPU, and a config needing more raises SlidingAttnError (SS_ERR_WORKSPACE_TOO_SMALL).  bf16 caches
+    only.  The binding itself allocates `out` only when the caller does not pass one - pass `out` to allocate nothing."""
+    lib = load()
+    if not (k_cache.is_cuda and k_cache.dtype == torch.bfloat16):
+        raise SlidingAttnError("k_cache: expected a CUDA bfloat16 tensor")
+    P, Hkv, page, D = k_cache.shape
+    _want(v_cache, "v_cache", torch.bfloat16, True, k_cache.shape)
+    R, T, Hq = ctx_lens.shape[0], q.shape[0], q.shape[1]
+    _want(q, "q", torch.bfloat16, True, (T, Hq, D))
+    _want(ctx_lens, "ctx_lens", torch.int32, True, (R,))
+    _want(query_start_loc, "query_start_loc", torch.int32, True, (R + 1,))
+    _want(block_table, "block_table", torch.int32, True, (R, block_table.shape[1]))
+    if out is None:
+        out = torch.empty_like(q)
+    _want(out, "out", torch.bfloat16, True, (T, Hq, D))
+    if lse is not None:
+        _want(lse, "lse", torch.float32, True)
+        if lse.numel() < T * Hq:
+            raise SlidingAttnError("lse: needs at least T * Hq elements")
+    cfg = ss_config(Hq, Hkv, D, page, P, max(max_requests or R, 1), max(max_tokens or T, 1), block_table.shape[1], 0)
+    msg = ctypes.create_string_buffer(512)
+    rc = lib.ss_mixed_attention_static(ctypes.byref(cfg), k_cache.data_ptr(), v_cache.data_ptr(), _ptr(q),
+                                       _ptr(block_table), _ptr(query_start_loc), _ptr(ctx_lens), R, T, float(scale),
+                                       _ptr(out), _ptr(lse), _stream_ptr(stream), msg, len(msg))
+    if rc != SS_OK:
+        err = SlidingAttnError(f"{lib.ss_status_string(rc).decode()} ({rc}) {msg.value.decode()}")
+        err.status = rc
+        raise err
+    return out
 
 
 def handle_for(batch, tensors, extra_tokens: int = 0, debug_checks: bool = False, fp8_caches=None, kv_scales=None) -> SlidingAttn:

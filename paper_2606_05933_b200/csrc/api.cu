@@ -39,13 +39,25 @@ int fail_cuda(Handle* h, cudaError_t e, const char* where) {
         if (e__ != cudaSuccess) return fail_cuda(h, e__, where); \
     } while (0)
 
+int check_batch_args(const Handle* h, const void* a, const void* b, const void* c, const void* d, int R, int T) {
+    if (!h) return SS_ERR_INVALID_ARG;
+    if (R < 0 || T < 0 || R > h->cfg.max_requests || T > h->cfg.max_tokens) return SS_ERR_INVALID_ARG;
+    if (R == 0 || T == 0) return SS_OK;
+    if (!a || !b || !c || !d) return SS_ERR_INVALID_ARG;
+    if (!aligned16(a) || !aligned16(b)) return SS_ERR_INVALID_ARG;
+    if ((((uintptr_t)c) & 3u) || (((uintptr_t)d) & 3u)) return SS_ERR_INVALID_ARG;
+    return SS_OK;
+}
+
+}  // namespace
+
 // KV cache [num_pages][Hkv][16][D] bf16 viewed as a 4-D tensor (innermost first): 64 columns of a 128-byte half row,
 // 8 rows of an 8-key group (stride D*2 bytes), D/64 halves (stride 128 bytes), 8-key groups (stride 8*D*2 bytes; a
 // (page, kv head) slab is two consecutive groups).  One TMA box = one whole slab: 2 groups x halves x 8 rows x 64
 // columns, written to shared memory as [group][half][8 rows][128 B] with SWIZZLE_128B - every [8 rows][128 B] block is a
 // canonical UMMA / ldmatrix core group, groups uniformly D/64 KB apart.  One operation per slab instead of one per
 // (slab, half): the per-SM copy engine costs ~31 ns per operation whatever its size (profiles/r2b.md).
-int encode_cache_map(Handle* h, CUtensorMap* map, void* base) {
+int ss::encode_cache_map(Handle* h, CUtensorMap* map, void* base) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) {
         snprintf(h->err, sizeof h->err, "cuTensorMapEncodeTiled entry point not found");
@@ -68,18 +80,6 @@ int encode_cache_map(Handle* h, CUtensorMap* map, void* base) {
     }
     return SS_OK;
 }
-
-int check_batch_args(const Handle* h, const void* a, const void* b, const void* c, const void* d, int R, int T) {
-    if (!h) return SS_ERR_INVALID_ARG;
-    if (R < 0 || T < 0 || R > h->cfg.max_requests || T > h->cfg.max_tokens) return SS_ERR_INVALID_ARG;
-    if (R == 0 || T == 0) return SS_OK;
-    if (!a || !b || !c || !d) return SS_ERR_INVALID_ARG;
-    if (!aligned16(a) || !aligned16(b)) return SS_ERR_INVALID_ARG;
-    if ((((uintptr_t)c) & 3u) || (((uintptr_t)d) & 3u)) return SS_ERR_INVALID_ARG;
-    return SS_OK;
-}
-
-}  // namespace
 
 extern "C" {
 

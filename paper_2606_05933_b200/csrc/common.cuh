@@ -134,6 +134,8 @@ cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_
                                     const int32_t* ctx, int R, int T, float scale, void* out, float* lse,
                                     cudaStream_t stream, int prefill_only = 0);
 bool main_self_plans(const Handle* h, int R, int T);
+// TMA descriptor of one cache tensor (api.cu; host-only encode, needs h->cfg / h->kv_fp8, writes h->err on failure)
+int encode_cache_map(Handle* h, CUtensorMap* map, void* base);
 cudaError_t init_main_attention(int head_dim, int kv_fp8);   // one-time function attributes (ss_create)
 // SS_FLAG_DEBUG_CHECKS: device-side validation of (qsl, ctx_lens, block_table); records the first violation in
 // h->state[kStateErr..] - the hot kernels of this and later calls then skip every cache / output access
