@@ -14,8 +14,12 @@ Pieces, in the paper's names:
   B*     = argmin_b T_hat(b) + T_hat(B_sigma - b),  B_sigma = B_cur + B_next         (Eq. 16)
            by the discrete ternary search of Algorithm 1 (stop at r - l <= 30, then compare {l0, r0, mid}).
 
-Readings of the garbled listing: line 9-15 = "if T1 <= T2 then r <- m2 - 1 else l <- m1 + 1"; a budget outside
-[|D|, B] in Pred(B_sigma - b) is clamped into that range (the paper does not say); ties go to the larger budget (line 23).
+Readings of the garbled listing: line 9-15 = "if T1 <= T2 then r <- m2 - 1 else l <- m1 + 1"; ties go to the larger
+budget (line 23).  The search range is the b for which BOTH windows get a budget an iteration can run,
+max(|D|, B_sigma - B) <= b <= min(B, B_sigma - |D|): "B_sigma - b [is] the approximate budget for the next window"
+(PAPER.md:210), so the two windows always carry B_sigma tokens between them.  (Round 2 searched [|D|, B] and clamped
+B_sigma - b instead; with plenty of slack, B_sigma = 2B, the clamped objective is smallest at b = |D| - it rewards
+dropping the prefill tokens rather than balancing them, and a calm system starved its prefill.  DESIGN.md reading 17.)
 """
 from __future__ import annotations
 
@@ -83,7 +87,7 @@ def sliding_chunker(F: BatchForwarder, decodes: Sequence[int], prefills: Sequenc
     b_cur = F.time_to_budget(decodes, prefills, t_cur)
     b_next = F.time_to_budget(decodes, prefills, t_next)
     b_sigma = b_cur + b_next
-    l, r = len(decodes), F.B
+    l, r = max(len(decodes), b_sigma - F.B), min(F.B, b_sigma - len(decodes))
     l0, r0 = l, r
     two = lambda b: F.pred(b, decodes, prefills) + F.pred(b_sigma - b, decodes, prefills)
     while r - l > stop_width:

@@ -201,10 +201,16 @@ def schedule_round(predict: Callable[[Sequence[Request]], float], max_budget: in
         return BatchDecision(len(dctx), len(dctx), {}, "decode_only",
                              predicted=predict([(1, u) for u in dctx]) if dctx else 0.0)
     risky, t_full, _ = violation_check(F, dctx, cands, t)                             # steps (3)-(4)
+    unsavable = []
     if risky:                                                                         # step (6)
         dec = batch_constructor(F, dctx, cands, t, eps)
-        if dec is not None:
+        # Algorithm 2 ends with its line-13 placeholder (B_dec, {}) when no at-risk anchor can still be saved this round
+        # (e.g. a request whose slack is already <= 0).  Running that as the round would repeat forever - the doomed
+        # request only gets riskier - and starve every healthy prefill behind it.  An empty Y* is therefore read as
+        # Algorithm 2's "no decision" and the round falls through to the SlidingChunker (reading 24).
+        if dec is not None and dec.prefill_alloc:
             return dec
+        unsavable = risky
     # step (5): SlidingChunker.  Protected decodes = all decodes (g_i = 1 for decoding requests)
     states = _states(cands)
     if decodes:
@@ -221,4 +227,4 @@ def schedule_round(predict: Callable[[Sequence[Request]], float], max_budget: in
     reqs = [(1, u) for u in dctx] + [(a, c.computed) for c, a in zip(cands, a_star) if a > 0]
     return BatchDecision(b_star, len(dctx), alloc, "sliding_chunker", predicted=predict(reqs) if reqs else 0.0,
                          info={"t_cur": t_cur, "t_next": t_next, "b_sigma": b_sigma, "t_two_window": t_star,
-                               "t_full": t_full})
+                               "t_full": t_full, "unsavable": unsavable})

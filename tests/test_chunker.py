@@ -53,8 +53,10 @@ def test_ternary_search_matches_brute_force_on_the_two_window_objective():
         assert abs(t_star - two(b_star)) < 1e-9
         # Algorithm 1 evaluates {l0, r0, mid of the final bracket}: never worse than both ends of the range, and within
         # the final bracket's resolution of the exhaustive optimum of the (here unimodal-or-flat) objective
-        best = min(two(b) for b in range(len(dec), F.B + 1))
-        assert t_star <= min(two(len(dec)), two(F.B)) + 1e-9
+        lo, hi = max(len(dec), b_sigma - F.B), min(F.B, b_sigma - len(dec))      # both windows get a runnable budget
+        assert lo <= b_star <= hi
+        best = min(two(b) for b in range(lo, hi + 1))
+        assert t_star <= min(two(lo), two(hi)) + 1e-9
         assert t_star - best <= 0.02 * best + 0.5
 
 
@@ -105,8 +107,10 @@ def test_chunker_on_the_measured_surface():
         assert sum(a_star) == min(b_star - len(dec), 5700) and a_star[0] == min(3800, b_star - len(dec))
         two = lambda b: F.pred(b, dec, pre) + F.pred(b_sigma - b, dec, pre)
         assert abs(t_star - two(b_star)) < 1e-9
-        assert t_star <= min(two(len(dec)), two(F.B)) + 1e-9
-        best = min(two(b) for b in range(len(dec), F.B + 1, 7))
+        lo_b, hi_b = max(len(dec), b_sigma - F.B), min(F.B, b_sigma - len(dec))
+        assert lo_b <= b_star <= hi_b
+        assert t_star <= min(two(lo_b), two(hi_b)) + 1e-9
+        best = min(two(b) for b in range(lo_b, hi_b + 1, 7))
         assert t_star - best <= 0.02 * best + 0.5
 
 
@@ -119,3 +123,12 @@ def test_fig1_example_runs_on_the_committed_surface():
     two = lambda b: F.pred(b, dec, pre) + F.pred(b_sigma - b, dec, pre)
     assert two(sliding[0]) <= two(single[0]) + 1e-9            # Eq. 16 on the unchanged (D, P)
     assert F.pred(single[0], dec, pre) <= t_cur and F.pred(single[1], dec, pre) <= t_next
+
+
+def test_plenty_of_slack_does_not_drop_the_prefill():
+    """With slack for two full iterations (B_sigma = 2B) the only split that keeps B_sigma tokens in two runnable
+    windows is b = B; the round-2 clamped objective chose b = |D| (decode only) here and starved the prefill."""
+    F = BatchForwarder(_toy_model, max_budget=1024)
+    dec, pre = [400 + i for i in range(8)], [PrefillState(900, 0), PrefillState(1500, 0)]
+    b_star, a_star, _, b_sigma = sliding_chunker(F, dec, pre, 1e6, 1e6)
+    assert b_sigma == 2048 and b_star == 1024 and a_star == [900, 116]

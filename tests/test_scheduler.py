@@ -171,3 +171,30 @@ def test_schedule_round_takes_the_right_branch():
     assert d2.predicted <= 8.0 + 1e-9                                # request 200's slack: -50 + 58 - 0
     d3 = schedule_round(_toy_model, 2048, decodes, [], [], t, rho=100.0)
     assert d3.branch == "decode_only" and d3.budget == 16
+
+
+def test_a_doomed_request_does_not_starve_healthy_prefill():
+    """a request that can no longer meet its TTFT (slack <= 0, so no anchor is feasible) makes Algorithm 2 end
+    on its empty placeholder every round.  The round must then fall through to the SlidingChunker so the healthy
+    requests behind it keep prefilling; simulated over several rounds."""
+    decodes = [DecodeRequest(i, ctx=400 + i, tbt_slo=40.0, last_token_time=0.0) for i in range(8)]
+    doomed = PrefillRequest(1, arrival=-100.0, ttft_slo=50.0, prompt_len=900)            # slack -50 at t = 0
+    healthy = [PrefillRequest(2, 0.0, 5000.0, 1500), PrefillRequest(3, 0.0, 5000.0, 700)]
+    reqs = {r.rid: r for r in [doomed] + healthy}
+    t, first = 0.0, None
+    for rnd in range(12):
+        waiting = [r for r in reqs.values() if r.remaining() > 0]
+        if not waiting:
+            break
+        for d in decodes:
+            d.last_token_time = t
+        dec = schedule_round(_toy_model, 1024, decodes, [], waiting, t, rho=100.0)
+        first = first or dec
+        assert dec.prefill_alloc, f"round {rnd}: prefill starved ({dec.branch})"
+        assert sum(dec.prefill_alloc.values()) + dec.decode_tokens <= dec.budget <= 1024
+        for rid, a in dec.prefill_alloc.items():
+            assert 0 < a <= reqs[rid].remaining()
+            reqs[rid].computed += a
+        t += dec.predicted
+    assert first.branch == "sliding_chunker" and first.info["unsavable"] == [1]
+    assert all(r.remaining() == 0 for r in reqs.values()), "every request, the doomed one included, finishes its prefill"
