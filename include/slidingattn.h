@@ -31,7 +31,7 @@
  *     SS_FLAG_DEBUG_CHECKS, page ids outside [0, num_pages), a query_start_loc that is not
  *     0 = qsl[0] <= ... <= qsl[R] = T, a negative ctx_len or ceil((u_r+c_r)/16) > max_pages_per_req are
  *     undefined behaviour.  With the flag, every ss_kv_append / ss_mixed_attention first runs a device-side
- *     check of exactly these conditions; on a violation it records (code, request, value) in a device flag
+ *     check of exactly these conditions (on FP8 handles also: every k_scale / v_scale entry finite and > 0); on a violation it records (code, request, value) in a device flag
  *     and the call - and every later call on the handle - touches neither the caches nor `out` until
  *     ss_poll_device_error has reported and cleared it.
  *   - ONE CALL IN FLIGHT PER HANDLE: the work-queue tickets and split-arrival counters are handle-owned

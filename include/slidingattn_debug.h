@@ -55,7 +55,8 @@ int ss_debug_force_simple_path(ss_handle* h, int on);
 
 /* Debug / tuning knobs; value 0 restores the automatic choice.  which: 1 = CTAs of the main launch (default one
  * per SM), 2 = number of CTAs that drain the decode queue first (default: balanced from the batch's decode bytes and
- * prefill flops by the planner; -1 = none), 3 = decode split length in keys (multiple of 128), 4 = nonzero forces the
+ * prefill flops by the planner; -1 = none), 3 = decode split length in keys (multiple of 128, within [512, 16384]; raised per batch until
+ * the splits fit the workspace's partial slots, which are sized for the automatic length), 4 = nonzero forces the
  * two-launch route (stand-alone work-list kernel + main kernel reading its items) that batches of more than 256
  * requests take; by default smaller batches are planned inside the main kernel (one launch).
  * Results never depend on these; only timing does.  SS_ERR_INVALID_ARG for an unknown key. */

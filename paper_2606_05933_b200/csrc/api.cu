@@ -227,7 +227,8 @@ int ss_debug_set_param(ss_handle* hh, int which, int value) {
     Handle* h = (Handle*)hh;
     if (!h || which < 1 || which >= 8) return SS_ERR_INVALID_ARG;
     if (which == kDbgSplitKeys && value > 0) {
-        // the workspace's partial slots are sized for split lengths in [kMinSplitKeys, kMaxSplitKeys]
+        // the workspace's item / partial slots are sized for the automatic split length; the plan raises a forced
+        // length until the batch's splits fit them (plan.cuh), so the knob can never write past the workspace
         value = (value + kTileKeys - 1) / kTileKeys * kTileKeys;
         if (value < kMinSplitKeys) value = kMinSplitKeys;
         if (value > kMaxSplitKeys) value = kMaxSplitKeys;
@@ -299,7 +300,7 @@ int ss_mixed_attention(ss_handle* hh, const void* q, const int32_t* block_table,
     if (h->force_simple) {
         SS_CUDA(h, launch_simple_attention(h, q, block_table, query_start_loc, ctx_lens, R, T, scale, out, lse_or_null, st),
                 "simple attention launch");
-        h->last_launches = 1;
+        h->last_launches = 1 + h->debug_checks;
         return SS_OK;
     }
     const bool two_kernels = !main_self_plans(h, R, T);
@@ -338,6 +339,7 @@ int ss_poll_device_error(ss_handle* hh, void* cuda_stream) {
                        : rec[0] == kChkCtxNegative  ? "negative ctx_len"
                        : rec[0] == kChkTooManyPages ? "ceil((u+c)/16) exceeds max_pages_per_req"
                        : rec[0] == kChkPageId       ? "block_table page id outside [0, num_pages)"
+                       : rec[0] == kChkKvScale      ? "FP8 k_scale / v_scale entry not finite and > 0 (request = kv head, + Hkv for v_scale; value = its bits)"
                                                     : "unknown check";
     snprintf(h->err, sizeof h->err, "device check %d: %s (request %d, value %d, limit %d)", rec[0], what, rec[1], rec[2], rec[3]);
     return SS_ERR_DEVICE_CHECK;

@@ -184,7 +184,7 @@ struct MixParams {
     // a2 inside this kernel (self_plan) or items read from the work-list kernel's output
     const int32_t* qsl;
     int32_t* queue;                // [0] next prefill ticket, [1] next decode ticket, [2] CTAs done (self_plan only)
-    int self_plan, R, num_sms, force_split_keys, force_decode_ctas;
+    int self_plan, R, num_sms, force_split_keys, force_decode_ctas, max_partials;
     unsigned long long* trace;     // ss_debug_set_trace: per-CTA timeline, or null
     int trace_words;
     const float* k_scale;          // SS_FLAG_KV_FP8: per kv head scales (device), else null
@@ -827,7 +827,7 @@ mixed_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__
     } else if (prm.self_plan) {
         // a2: every CTA builds the same plan (scratch = the still unused K ring); items are decoded from queue tickets
         build_plan<MixCta<FP8>::kThreads, uint16_t>(prm.qsl, prm.ctx_lens, prm.R, Hq, Hkv, D, prm.num_sms, prm.force_split_keys,
-                                          prm.force_decode_ctas, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph);
+                                          prm.force_decode_ctas, prm.max_partials, reinterpret_cast<int32_t*>(smem + SM::kKOff), ptb, ph);
         fence_proxy_async();    // scratch was written through the generic proxy; TMA writes the same bytes next
     } else if (threadIdx.x == 0) {
         ph->tot_p = prm.hdr->n_prefill;
@@ -1404,6 +1404,7 @@ cudaError_t launch_main_attention(const Handle* h, const void* q, const int32_t*
     p.num_sms = h->num_sms;
     p.force_split_keys = h->dbg[kDbgSplitKeys];
     p.force_decode_ctas = h->dbg[kDbgDecodeCtas];
+    p.max_partials = h->ws.max_partials;
     p.partials = (float*)(ws + h->ws.partial_off);
     p.q = (const __nv_bfloat16*)q;
     p.out = (__nv_bfloat16*)out;

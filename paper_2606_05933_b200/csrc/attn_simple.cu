@@ -30,8 +30,9 @@ simple_attention_kernel(const __nv_bfloat16* __restrict__ q, const void* __restr
                         const float* __restrict__ v_scale, const int32_t* __restrict__ block_table,
                         const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int T,
                         int Hq, int Hkv, int max_pages, float scale, __nv_bfloat16* __restrict__ out,
-                        float* __restrict__ lse, int prefill_only) {
+                        float* __restrict__ lse, int prefill_only, const int32_t* __restrict__ err_flag) {
     constexpr int EPL = D / 32;                       // output elements per lane
+    if (err_flag && *reinterpret_cast<const volatile int32_t*>(err_flag) != 0) return;   // tripped debug check: touch nothing
     __shared__ float s_q[4][D];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t unit = (int64_t)blockIdx.x * 4 + warp;   // (row, head)
@@ -138,18 +139,19 @@ cudaError_t launch_simple_attention(const Handle* h, const void* q, const int32_
     const ss_config& c = h->cfg;
     const int64_t units = (int64_t)T * c.num_q_heads;
     const unsigned blocks = (unsigned)((units + 3) / 4);
+    const int32_t* err = h->debug_checks ? h->state + kStateErr : nullptr;
     if (h->kv_fp8)
         simple_attention_kernel<128, true><<<blocks, 128, 0, stream>>>(
             (const __nv_bfloat16*)q, h->k_cache, h->v_cache, h->k_scale, h->v_scale, bt, qsl, ctx, R, T, c.num_q_heads,
-            c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
+            c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only, err);
     else if (c.head_dim == 128)
         simple_attention_kernel<128, false><<<blocks, 128, 0, stream>>>(
             (const __nv_bfloat16*)q, h->k_cache, h->v_cache, nullptr, nullptr, bt, qsl, ctx, R, T, c.num_q_heads,
-            c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
+            c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only, err);
     else
         simple_attention_kernel<64, false><<<blocks, 128, 0, stream>>>(
             (const __nv_bfloat16*)q, h->k_cache, h->v_cache, nullptr, nullptr, bt, qsl, ctx, R, T, c.num_q_heads,
-            c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only);
+            c.num_kv_heads, c.max_pages_per_req, scale, (__nv_bfloat16*)out, lse, prefill_only, err);
     return cudaGetLastError();
 }
 

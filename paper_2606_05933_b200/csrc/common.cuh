@@ -50,7 +50,7 @@ struct WorkspaceLayout {
 constexpr int kStateErr = 4;         // Handle::state word offsets
 constexpr int kStateCounters = 8;
 // debug-check codes (ss_poll_device_error)
-enum { kChkQsl = 1, kChkCtxNegative = 2, kChkTooManyPages = 3, kChkPageId = 4 };
+enum { kChkQsl = 1, kChkCtxNegative = 2, kChkTooManyPages = 3, kChkPageId = 4, kChkKvScale = 5 };
 
 struct Handle {
     ss_config cfg;

@@ -53,8 +53,8 @@ __device__ __forceinline__ int plan_decode_chunk(int n, int L) {
 // (u + c < 2^29).
 template <int NT, typename OffT>
 __device__ void build_plan(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int Hq, int Hkv,
-                           int D, int num_sms, int force_split_keys, int force_decode_ctas, int32_t* scratch,
-                           PlanTables<OffT> tb, PlanHeader* ph) {
+                           int D, int num_sms, int force_split_keys, int force_decode_ctas, int max_decode_items,
+                           int32_t* scratch, PlanTables<OffT> tb, PlanHeader* ph) {
     int32_t* s_c = scratch;
     int32_t* s_u = scratch + R;
     int32_t* s_cost = scratch + 2 * ((R + 3) & ~3);          // 16-byte aligned: read as int4
@@ -93,7 +93,15 @@ __device__ void build_plan(const int32_t* __restrict__ qsl, const int32_t* __res
         L = (L + kTileKeys - 1) / kTileKeys * kTileKeys;
         if (L < (unsigned long long)kMinSplitKeys) L = kMinSplitKeys;
         if (L > (unsigned long long)kMaxSplitKeys) L = kMaxSplitKeys;
-        if (force_split_keys > 0) L = (unsigned long long)(force_split_keys + kTileKeys - 1) / kTileKeys * kTileKeys;
+        if (force_split_keys > 0) {
+            L = (unsigned long long)(force_split_keys + kTileKeys - 1) / kTileKeys * kTileKeys;
+            // The workspace's item / partial slots are sized for the automatic L (workspace_layout).  A forced, shorter L
+            // can ask for more: sum_r ceil(n_r / L) <= total_keys / L + nD splits per kv head.  Raise it until the batch
+            // fits; at kMaxSplitKeys it always does.
+            while (L < (unsigned long long)kMaxSplitKeys &&
+                   (ph->total_keys / L + (unsigned long long)ph->nD) * (unsigned long long)Hkv > (unsigned long long)max_decode_items)
+                L += kTileKeys;
+        }
         ph->L = (int)L;
     }
     __syncthreads();

@@ -5,6 +5,8 @@
 //   kChkCtxNegative   ctx_lens[r] >= 0
 //   kChkTooManyPages  ceil((u_r + c_r) / 16) <= max_pages_per_req            (requests with c_r > 0)
 //   kChkPageId        0 <= block_table[r][p] < num_pages for every page p < ceil((u_r + c_r) / 16)
+//   kChkKvScale       FP8 handles: k_scale[g], v_scale[g] finite and > 0 (value = the scale's bit pattern; request = g for
+//                     k_scale, Hkv + g for v_scale) - the kernels' running max of raw scores needs k_scale > 0
 // The first violation wins (atomicCAS on the code word) and records (code, request, offending value, limit).  The hot
 // kernels read the code word after their grid-dependency wait and, if it is set, touch neither caches nor outputs;
 // the flag stays set until ss_poll_device_error clears it.  Integer work only.
@@ -25,10 +27,16 @@ __device__ __forceinline__ void report(int32_t* err, int code, int req, long lon
 
 __global__ void __launch_bounds__(kValThreads)
 validate_kernel(const int32_t* __restrict__ block_table, const int32_t* __restrict__ qsl,
-                const int32_t* __restrict__ ctx_lens, int R, int T, int max_pages, long long num_pages, int32_t* err) {
+                const int32_t* __restrict__ ctx_lens, int R, int T, int max_pages, long long num_pages, int32_t* err,
+                const float* __restrict__ k_scale, const float* __restrict__ v_scale, int Hkv) {
     ptx::pdl_wait();
     const int warp = (blockIdx.x * kValThreads + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     const int nwarps = gridDim.x * (kValThreads / 32);
+    if (k_scale && blockIdx.x == 0)
+        for (int i = threadIdx.x; i < 2 * Hkv; i += kValThreads) {
+            const float s = i < Hkv ? __ldg(k_scale + i) : __ldg(v_scale + i - Hkv);
+            if (!(s > 0.f) || !(s <= 3.4028234e38f)) report(err, kChkKvScale, i, (long long)__float_as_int(s), 0);   // NaN fails both
+        }
     if (warp == 0 && lane == 0) {
         if (__ldg(qsl) != 0) report(err, kChkQsl, 0, __ldg(qsl), 0);
         if (__ldg(qsl + R) != T) report(err, kChkQsl, R, __ldg(qsl + R), T);
@@ -57,7 +65,8 @@ cudaError_t launch_validate(const Handle* h, const int32_t* bt, const int32_t* q
     if (grid > 4 * h->num_sms) grid = 4 * h->num_sms;
     if (grid < 1) grid = 1;
     validate_kernel<<<grid, kValThreads, 0, stream>>>(bt, qsl, ctx, R, T, h->cfg.max_pages_per_req,
-                                                      (long long)h->cfg.num_pages, h->state + kStateErr);
+                                                      (long long)h->cfg.num_pages, h->state + kStateErr,
+                                                      h->kv_fp8 ? h->k_scale : nullptr, h->v_scale, h->cfg.num_kv_heads);
     return cudaGetLastError();
 }
 

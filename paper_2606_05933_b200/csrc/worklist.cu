@@ -14,7 +14,8 @@ constexpr int kWlCtas = 8;            // every CTA rebuilds the (small) plan and
 __global__ void __launch_bounds__(kWlThreads)
 worklist_kernel(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx_lens, int R, int Hq, int Hkv,
                 int num_sms, int D, int force_split_keys, int force_decode_ctas, WorkHeader* __restrict__ hdr,
-                ss_work_item* __restrict__ items, int32_t* __restrict__ merge_counters, int max_items) {
+                ss_work_item* __restrict__ items, int32_t* __restrict__ merge_counters, int max_items,
+                int max_decode_items, const int32_t* __restrict__ err_flag) {
     extern __shared__ __align__(16) int32_t sm[];
     const int Rp = (R + 3) & ~3;
     int32_t* scratch = sm;                                        // 3 Rp
@@ -26,7 +27,11 @@ worklist_kernel(const int32_t* __restrict__ qsl, const int32_t* __restrict__ ctx
 
     ptx::pdl_launch_dependents();
     ptx::pdl_wait();            // qsl / ctx_lens may come from the preceding kernel in the stream
-    build_plan<kWlThreads, int32_t>(qsl, ctx_lens, R, Hq, Hkv, D, num_sms, force_split_keys, force_decode_ctas, scratch, tb, &ph);
+    // SS_FLAG_DEBUG_CHECKS: a tripped check means the metadata is not to be trusted (a negative ctx_len would divide by
+    // zero in the plan); like the append and main kernels, do nothing until ss_poll_device_error has cleared the flag
+    if (err_flag && *reinterpret_cast<const volatile int32_t*>(err_flag) != 0) return;
+    build_plan<kWlThreads, int32_t>(qsl, ctx_lens, R, Hq, Hkv, D, num_sms, force_split_keys, force_decode_ctas, max_decode_items,
+                                    scratch, tb, &ph);
     if (blockIdx.x == 0)
         for (int i = tid; i < R * Hkv; i += nt) merge_counters[i] = 0;     // "last split merges" arrival counters
     const int total = ph.tot_p + ph.tot_d;
@@ -60,7 +65,8 @@ cudaError_t launch_worklist(const Handle* h, const int32_t* qsl, const int32_t* 
     return launch_pdl(worklist_kernel, dim3(kWlCtas), dim3(kWlThreads), smem, stream, qsl, ctx, R, h->cfg.num_q_heads,
                       h->cfg.num_kv_heads, h->num_sms, h->cfg.head_dim, h->dbg[kDbgSplitKeys], h->dbg[kDbgDecodeCtas],
                       (WorkHeader*)(ws + w.header_off), (ss_work_item*)(ws + w.items_off),
-                      (int32_t*)(ws + w.counters_off), w.max_items);
+                      (int32_t*)(ws + w.counters_off), w.max_items, w.max_partials,
+                      (const int32_t*)(h->debug_checks ? h->state + kStateErr : nullptr));
 }
 
 }  // namespace ss

@@ -221,6 +221,34 @@ def test_fp8_needs_scales_and_head_dim_128():
     assert ei.value.status == binding.SS_ERR_INVALID_ARG
 
 
+def test_fp8_debug_checks_catch_bad_scales():
+    """the header says every FP8 scale is finite and > 0; with SS_FLAG_DEBUG_CHECKS the device check now
+    enforces it (a zero or negative k_scale breaks the running max of the raw scores silently)."""
+    b = wl.make_batch("fp8-scales", 8, 2, 128, [(1, 300), (40, 10)], 81, with_append=True)
+    t = wl.make_tensors(b, DEV)
+    ks, vs = fp8_scales(2, 7)
+    kc, vc = quantise_pool(t.k_cache, ks), quantise_pool(t.v_cache, vs)
+    k_dev, v_dev = dev(ks), dev(vs)
+    h = binding.handle_for(b, t, fp8_caches=(kc, vc), kv_scales=(k_dev, v_dev), debug_checks=True)
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    kc0 = kc.clone()
+    for which, idx, bad in ((k_dev, 1, 0.0), (k_dev, 0, -0.01), (v_dev, 1, float("nan")), (v_dev, 0, float("inf"))):
+        good = float(which[idx])
+        which[idx] = bad
+        out = torch.full_like(t.q, 7.0)
+        binding.kv_append(h, t.k_new, t.v_new, bt, qsl, ctx)
+        binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale, out=out)
+        with pytest.raises(binding.SlidingAttnError, match="device check 5") as ei:
+            h.poll_device_error()
+        assert f"request {idx + (2 if which is v_dev else 0)}," in str(ei.value)
+        assert torch.equal(kc, kc0) and bool((out == 7.0).all())
+        which[idx] = good
+    binding.kv_append(h, t.k_new, t.v_new, bt, qsl, ctx)
+    out = binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale, out=torch.full_like(t.q, float("nan")))
+    h.poll_device_error()
+    assert not torch.isnan(out.float()).any() and not torch.equal(kc, kc0)
+
+
 def test_fp8_bitwise_reproducible_whatever_ran_before():
     """The split of an item's keys between the decode warpgroups must not depend on the CTA's history (dynamic queue):
     repeated calls, and the same batch after a different batch on the same handle, give identical bits."""

@@ -524,6 +524,77 @@ def test_debug_checks_flag_bad_metadata_and_skip_the_access():
     assert h.last_launch_count() == 2                 # validate + main launch
 
 
+@pytest.mark.parametrize("route", ["more requests than the in-kernel plan holds", "knob 4", "simple path"])
+def test_debug_checks_cover_the_two_launch_route_and_the_simple_path(route):
+    """the stand-alone work-list kernel and the warp-per-row kernel must also stand still after a tripped
+    check (a negative ctx_len would otherwise divide by zero in the plan / walk a bad page id), the launch count
+    includes the validate launch on every route, and the handle serves a good batch afterwards."""
+    if route == "more requests than the in-kernel plan holds":
+        reqs = [(1, 40 + 3 * i) for i in range(280)] + [(70, 100), (1, 2000)]
+    else:
+        reqs = [(1, 900), (130, 64), (1, 0), (1, 3000), (40, 0)]
+    b = wl.make_batch("dbg-routes", 8, 2, 128, reqs, 93, with_append=False)
+    t = wl.make_tensors(b, DEV)
+    h = binding.handle_for(b, t, debug_checks=True)
+    if route == "knob 4":
+        h.debug_set_param(4, 1)
+    h.force_simple_path(route == "simple path")
+    bt, qsl = dev(b.block_table), dev(b.query_start_loc)
+    neg_ctx = b.ctx_lens.copy()
+    neg_ctx[1] = -5
+    bad_bt = b.block_table.copy()
+    bad_bt[3, 0] = b.num_pages + 7
+    for ctx_h, bt_h, code in ((neg_ctx, b.block_table, 2), (b.ctx_lens, bad_bt, 4)):
+        out = torch.full_like(t.q, 7.0)
+        binding.mixed_attention(h, t.q, dev(bt_h), qsl, dev(ctx_h), b.scale, out=out)
+        with pytest.raises(binding.SlidingAttnError, match=f"device check {code}"):
+            h.poll_device_error()
+        assert bool((out == 7.0).all()), "out written after a tripped check"
+    out = torch.full_like(t.q, float("nan"))
+    binding.mixed_attention(h, t.q, bt, qsl, dev(b.ctx_lens), b.scale, out=out)
+    h.poll_device_error()
+    assert h.last_launch_count() == (2 if route == "simple path" else 3)    # validate (+ work list) + attention
+    ref, _ = oracle_run_from_device(b, t)
+    check(b, out, ref)
+
+
+@pytest.mark.parametrize("two_launch", [False, True])
+def test_forced_short_split_never_outgrows_the_workspace(two_launch):
+    """the workspace's partial slots are sized for the automatic split length.  Forcing 512-key splits on a
+    few very long contexts asks for ~10x more items than there are slots; the plan must raise the length until they
+    fit instead of writing past the workspace.  A guard buffer right behind the workspace must stay untouched and the
+    result must not depend on the knob."""
+    reqs = [(1, 60000), (1, 52345), (1, 7), (1, 33000), (150, 20000)]
+    b = wl.make_batch("forced-L", 32, 8, 128, reqs, 94, with_append=False)
+    t = wl.make_tensors(b, DEV)
+    bt, qsl, ctx = dev(b.block_table), dev(b.query_start_loc), dev(b.ctx_lens)
+    h = binding.handle_for(b, t)
+    ref_out = binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale).clone()
+    # the handle's workspace, re-seated at the front of a larger buffer whose tail is the guard
+    guard_bytes = 8 << 20
+    big = torch.full((h.workspace_bytes + guard_bytes,), 0x5A, dtype=torch.uint8, device=DEV)
+    h.workspace = big
+    h.debug_set_param(3, 512)
+    if two_launch:
+        h.debug_set_param(4, 1)
+    out = binding.mixed_attention(h, t.q, bt, qsl, ctx, b.scale, out=torch.full_like(t.q, float("nan")))
+    torch.cuda.synchronize()
+    assert bool((big[h.workspace_bytes:] == 0x5A).all()), "wrote past the workspace"
+    items, counts = h.build_worklist(qsl, ctx)
+    splits = items[items["kind"] == 2]
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    slots = 8 * b.R * (-(-b.max_pages_per_req * 16 // 16384) + 1) + sms + 64          # workspace_layout's max_partials
+    assert 8 * 512 * 8 * len(splits) > 145000 * 8, "the forced length was not honoured at all"
+    assert len(splits) > 5 * 8 and counts[2] <= slots                                 # still split, and inside the slots
+    assert bool((big[h.workspace_bytes:] == 0x5A).all())
+    g, r = out.to(torch.float64).cpu().numpy(), ref_out.to(torch.float64).cpu().numpy()
+    assert not np.isnan(g).any()
+    assert np.abs(g - r).max() <= MAX_ABS and np.abs(g - r).mean() <= MEAN_ABS
+    rows = np.asarray([0, 1, 3, 4, 153], dtype=np.int32)
+    ref, _ = oracle_run_from_device(b, t, rows=rows)
+    check(b, out, ref, rows=rows)
+
+
 def test_poll_is_clean_without_debug_checks_and_reset_rearms_the_handle():
     b = wl.random_batch(78, Hq=8, Hkv=2, D=128, n_prefill=1, n_decode=5, max_c=100, max_u=3000, with_append=False)
     t = wl.make_tensors(b, DEV)
