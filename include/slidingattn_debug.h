@@ -50,6 +50,11 @@ int ss_last_launch_count(const ss_handle* h);
 int ss_set_kernel_timing(ss_handle* h, int on);
 int ss_last_kernel_time_us(ss_handle* h, float* main_us);
 
+/* Measurement aid: one read-only streaming pass (16 KB bulk copies into shared memory, whole chunks only) over `bytes` of device memory at `buf` (16-byte aligned), enqueued on
+ * the stream.  bench.py times it to get the HBM READ peak of this GPU: the decode path only reads, and the copy
+ * (read + write) peak in MEASURED_PEAKS.json understates what a read-only stream can reach.  Touches no library state. */
+int ss_debug_stream_read(ss_handle* h, const void* buf, size_t bytes, void* cuda_stream);
+
 /* Debug: force the plain one-warp-per-row CUDA kernel (no tensor cores) for every row. 0 = off. */
 int ss_debug_force_simple_path(ss_handle* h, int on);
 

@@ -26,7 +26,8 @@ EXPORTS = ["ss_version", "ss_status_string", "ss_last_error_string", "ss_create"
            "ss_poll_device_error", "ss_reset"]
 # ... and include/slidingattn_debug.h (test / tuning / measurement aids)
 DEBUG_EXPORTS = ["ss_build_worklist", "ss_last_launch_count", "ss_debug_force_simple_path",
-                 "ss_debug_set_param", "ss_debug_set_trace", "ss_set_kernel_timing", "ss_last_kernel_time_us"]
+                 "ss_debug_set_param", "ss_debug_set_trace", "ss_set_kernel_timing", "ss_last_kernel_time_us",
+                 "ss_debug_stream_read"]
 
 
 class ss_config(ctypes.Structure):
@@ -84,6 +85,7 @@ def load():
     lib.ss_debug_force_simple_path.argtypes = [vp, ctypes.c_int]
     lib.ss_debug_set_param.argtypes = [vp, ctypes.c_int, ctypes.c_int]
     lib.ss_debug_set_trace.argtypes = [vp, vp, i32]
+    lib.ss_debug_stream_read.argtypes = [vp, vp, ctypes.c_size_t, vp]
     lib.ss_set_kernel_timing.argtypes = [vp, ctypes.c_int]
     lib.ss_last_kernel_time_us.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     for name in EXPORTS + DEBUG_EXPORTS:
@@ -272,6 +274,12 @@ class SlidingAttn:
         """1 = main-launch CTAs, 2 = decode-first CTAs, 3 = decode split keys, 4 = force the two-launch route; 0 = automatic."""
         self._check(self.lib.ss_debug_set_param(self._h, int(which), int(value)))
 
+
+    def stream_read(self, buf: torch.Tensor, stream=None):
+        """Measurement aid: one read-only streaming pass over a contiguous CUDA tensor (bench.py's HBM read peak)."""
+        assert buf.is_cuda and buf.is_contiguous()
+        self._check(self.lib.ss_debug_stream_read(self._h, buf.data_ptr(), buf.numel() * buf.element_size(),
+                                                  _stream_ptr(stream)))
 
     def set_trace(self, buf: Optional[torch.Tensor], words_per_cta: int = 0):
         """Per-CTA timeline of the main launch into a CUDA int64 tensor [num_ctas, words_per_cta]; None = off."""
