@@ -124,7 +124,8 @@ int ss_kv_append(ss_handle* h, const void* k_new, const void* v_new, const int32
  * heads.  q and k are rotated by the token's absolute position ctx_lens[r] + j with the "rotate-half" rotary embedding
  * of the model families the paper serves (reading 22):
  *     angle_i = pos * rope_theta^(-2i/D);  y_i = x_i cos - x_{i+D/2} sin;  y_{i+D/2} = x_{i+D/2} cos + x_i sin
- * (cos / sin evaluated in double, the rotation in fp32, one rounding to bf16).  Rotated q -> q_out [T][Hq][D] (the q
+ * (cos / sin and the rotation evaluated in double, products and sums rounded separately, ONE rounding to bf16: bit-exact
+ * against that definition up to the last place of cos / sin).  Rotated q -> q_out [T][Hq][D] (the q
  * argument of ss_mixed_attention), rotated k and the untouched v bits -> their page slots exactly as ss_kv_append places
  * them.  Replaces ss_kv_append for the batch.  rope_theta must be finite and > 1.  All pointers device.
  */

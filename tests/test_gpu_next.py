@@ -27,17 +27,14 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).to(DEV)
 
 
-def assert_within_one_bf16_ulp(got_u16, want_u16, what):
-    g, w = u16_to_f64(got_u16), u16_to_f64(want_u16)
-    odd = ~np.isfinite(w)                                   # poisoned unused slots (NaN payloads): must be untouched bits
-    assert np.array_equal(got_u16[odd], want_u16[odd]), f"{what}: non-finite patterns differ"
-    g, w = np.where(odd, 0.0, g), np.where(odd, 0.0, w)
-    assert np.isfinite(g).all(), f"{what}: non-finite values"
-    diff = np.abs(g - w)
-    ulp = np.maximum(np.abs(g), np.abs(w)) * 2.0 ** -7 + 3e-6
-    assert (diff <= ulp).all(), f"{what}: more than one bf16 ulp (+ 3e-6) apart (max {diff.max():.3e})"
-    frac = float((got_u16 != want_u16).mean())
-    assert frac < 2e-3, f"{what}: {frac:.2%} of the elements differ"
+def assert_same_bf16_bits(got_u16, want_u16, what):
+    """Round 3: the fused RoPE rotates in double with separately rounded products and one rounding to bf16 - the
+    oracle's arithmetic (reading 25) - so the comparison is bit for bit, unused (poisoned) slots included.
+    Only cos / sin come from another libm; their last-ulp differences can flip a bf16 rounding with probability
+    ~2^-44 per element."""
+    bad = got_u16 != want_u16
+    assert not bad.any(), (f"{what}: {int(bad.sum())} of {bad.size} elements differ from the oracle, first at "
+                           f"{tuple(int(i) for i in np.argwhere(bad)[0])}")
 
 
 def check_attention(b, out_gpu, ref):
@@ -66,8 +63,8 @@ def rope_case(b, theta):
     torch.cuda.synchronize()
     q_ref = oracle.rope_qkv_append(wl.to_u16(qkv), k0, v0, b.block_table, b.query_start_loc, b.ctx_lens, b.num_q_heads, theta)
     assert np.array_equal(wl.to_u16(t.v_cache), v0), "v_cache: the fused append must copy V bit for bit"
-    assert_within_one_bf16_ulp(wl.to_u16(q_rot), q_ref, "rotated q")
-    assert_within_one_bf16_ulp(wl.to_u16(t.k_cache), k0, "k_cache (rotated k; untouched slots identical)")
+    assert_same_bf16_bits(wl.to_u16(q_rot), q_ref, "rotated q")
+    assert_same_bf16_bits(wl.to_u16(t.k_cache), k0, "k_cache (rotated k; untouched slots identical)")
     ref, _, _ = oracle.mixed_attention(q_ref, k0, v0, b.block_table, b.query_start_loc, b.ctx_lens, b.scale)
     if b.T:
         check_attention(b, out, ref)
@@ -364,8 +361,8 @@ def test_randomized_shapes_and_mixes_bf16_and_fp8():
 def test_fp8_rope_qkv_append(shape, model):
     """Fused RoPE + QKV split over an FP8 cache: q as on a bf16 handle; k rotated and rounded to bf16 once, THEN quantised
     like ss_kv_append; v quantised.  Oracle = its RoPE append into scratch bf16 caches, then its FP8 append of those bits.
-    V codes bit-exact.  K codes: the kernel's fp32 rotation may land one bf16 ulp from the oracle's double rotation in
-    < 0.2 % of the elements (test above), so a code may differ there - by at most one E4M3 step, in < 0.5 % of them."""
+    q, K codes and V codes bit-exact (round 3: the rotation is the oracle's double arithmetic, so the bf16 value that
+    gets quantised is the oracle's)."""
     Hq, Hkv, D = shape
     b = wl.random_batch(5100 + Hq, Hq=Hq, Hkv=Hkv, D=D, n_prefill=2, n_decode=6, max_c=180, max_u=900)
     b = wl.Batch(**{**b.__dict__, "with_append": True})
@@ -389,14 +386,9 @@ def test_fp8_rope_qkv_append(shape, model):
             pos = u + j
             k_rot[int(b.query_start_loc[r]) + j] = sk[int(b.block_table[r][pos // 16]), :, pos % 16, :]
     oracle.kv_append_fp8(k0, v0, k_rot, wl.to_u16(t.v_new), ks, vs, b.block_table, b.query_start_loc, b.ctx_lens)
-    assert_within_one_bf16_ulp(wl.to_u16(q_rot), q_ref, "rotated q")
+    assert_same_bf16_bits(wl.to_u16(q_rot), q_ref, "rotated q")
     assert np.array_equal(vc.cpu().numpy(), v0), "FP8 v codes differ"
-    kg = kc.cpu().numpy()
-    diff = kg != k0
-    assert diff.mean() < 5e-3, f"{diff.mean():.3%} of the k codes differ"
-    a, bb = oracle.e4m3_to_f64(kg[diff]), oracle.e4m3_to_f64(k0[diff])
-    assert np.all(np.abs(a - bb) <= np.maximum(np.abs(a), np.abs(bb)) * 0.125 + 2.0 ** -9), "a k code is off by more than one E4M3 step"
-    # attention: the oracle on ITS OWN q and codes (nothing the CUDA path produced); the few one-step code differences stay
-    # far inside north_star's bounds
+    assert np.array_equal(kc.cpu().numpy(), k0), "FP8 k codes differ"
+    # attention: the oracle on ITS OWN q and codes (nothing the CUDA path produced)
     ref, _ = oracle.mixed_attention_fp8(q_ref, k0, v0, ks, vs, b.block_table, b.query_start_loc, b.ctx_lens, b.scale)
     check_attention(b, out, ref)
