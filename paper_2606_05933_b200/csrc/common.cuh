@@ -13,7 +13,7 @@
 namespace ss {
 
 constexpr int kPage = 16;             // tokens per KV page (BASELINE.json configs: "page 16")
-constexpr int kTileKeys = 128;        // keys per staged KV tile / MMA N
+constexpr int kTileKeys = 128;        // keys per prefill KV step (MMA N; two 64-key ring slots) and the alignment of decode splits
 constexpr int kTileRows = 128;        // query rows per prefill tile / MMA M
 constexpr int kMaxGroup = 16;         // max q heads per kv head on the decode path (MMA M = 16)
 constexpr int kDecodeWaves = 1;       // target decode items per SM when choosing the split length (a split costs ~2 us of
@@ -59,7 +59,7 @@ struct Handle {
     int group;                       // Hq / Hkv
     void* k_cache;
     void* v_cache;
-    CUtensorMap tmap_k, tmap_v;      // [pages*Hkv*16 rows][D] bf16, box 16 x 64, 128B swizzle
+    CUtensorMap tmap_k, tmap_v;      // 4-D slab maps, one box = one (page, kv head) slab, 128B swizzle (encode_cache_map, api.cu)
     bool have_tmaps;
     WorkspaceLayout ws;
     // host-iteration staging (lazy)
